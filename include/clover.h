@@ -1,0 +1,131 @@
+/*
+ * include/clover.h -- C-ABI of the B200-native Wilson-clover solve path of arXiv:1405.4524.
+ *
+ * What the calls compute (citations: P:L<n> = PAPER.md line n; S = SURVEY.md; R<n> = reading n in DESIGN.md):
+ *   The paper's stochastic propagators need, for every random source eta_r, the solution vector
+ *   X_r of  D X_r = eta_r  ("X is the solution vector and eta is the random source vector", P:L303,
+ *   eq. 7.3 at P:L300), D being "the lattice fermion matrix computed in the background of the gauge
+ *   fields" for "clover fermions with tree-level improved clover coefficient"; the paper
+ *   hands this to a GPU inverter through an interface that "just involved some reordering of the arrays"
+ *   (P:L318).  This library is that inverter and that interface.  The operator is
+ *       D = A - kappa H,
+ *       (H psi)(x) = sum_mu [ f_mu(x) (1 - gamma_mu) U_mu(x) psi(x+mu) + g_mu(x) (1 + gamma_mu) U_mu(x-mu)^+ psi(x-mu) ],
+ *       A(x) = 1 + i c_sw kappa sum_{mu<nu} sigma_{mu nu} (x) Fhat_{mu nu}(x),
+ *   with the gamma basis, boundary phases f, g and the four-leaf clover Fhat of S 8(c) O1-O4 (R1-R5).
+ *
+ * Canonical (ABI) layouts.  All arrays are C-ordered, complex numbers are (re, im) pairs:
+ *   links    double [4 mu][T][Z][Y][X][3 row][3 col][2]     U_mu(x) stored at x, pointing x -> x+mu
+ *   spinors  real   [n_rhs][T][Z][Y][X][4 spin][3 colour][2]   real = double, or float where a
+ *                                                               `precision` argument says 32
+ *   mu = 0,1,2,3 = x,y,z,t; dims = {X,Y,Z,T}, every extent even and >= 2; bc[mu] = +1 | -1.
+ *
+ * Pointers: every pointer named *_dev is a DEVICE pointer owned by the caller (e.g. torch tensor
+ * data_ptr()); *_host is HOST memory (pinned for full copy speed).  `stream` is a cudaStream_t cast
+ * to void* (NULL = legacy default stream).  The library never frees or keeps caller buffers: a
+ * context copies what it needs during clover_create.  Workspaces are owned by the context.
+ *
+ * Errors: every call returns 0 on success or a negative CLOVER_E* code (no exceptions, no abort, no
+ * printing).  clover_solve* additionally returns the positive count of right-hand sides that did
+ * not converge.  clover_last_error() gives a message for the last failure on the calling thread.
+ * There is no CPU fallback anywhere: without a CUDA device every call fails with CLOVER_ECUDA.
+ */
+#ifndef CLOVER_B200_H
+#define CLOVER_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CLOVER_OK 0
+#define CLOVER_EINVAL (-1) /* bad dims / odd extent / n_rhs out of range / null pointer / bad enum */
+#define CLOVER_ECUDA (-2)  /* a CUDA runtime call failed (message has the CUDA error string)        */
+#define CLOVER_ENOMEM (-3) /* device allocation failed                                              */
+
+typedef struct clover_ctx clover_ctx; /* opaque: reordered links, A, A^-1 (fp64 + fp32), workspaces */
+
+typedef struct {
+    int recon;   /* gauge storage of the fp32 (sloppy) links: 18 = full, 12 = two rows (third row rebuilt in-kernel).
+                    fp64 links are always stored in full. */
+    int max_rhs; /* largest batch any later call uses (1..8); sizes the workspaces */
+} clover_opts;
+
+typedef struct {
+    int status;           /* 0 converged, 1 max_iter reached, 2 breakdown, 3 non-finite */
+    int iters;            /* BiCGStab iterations of the batch this source was in */
+    int reliable_updates; /* fp64 residual recomputations of that batch */
+    double iter_resid;    /* last fp64 even-odd residual ||b_e - Mhat y|| / ||eta|| */
+    double true_resid;    /* full-lattice fp64 ||eta - D psi|| / ||eta||, recomputed from the returned psi */
+} clover_rhs_info;
+
+/* operators of dslash_apply (S 8(a) H3, H4; S 8(b)) */
+enum {
+    CLOVER_OP_HOP_EO = 0,     /* out_even = H in_odd,  out_odd = 0 */
+    CLOVER_OP_HOP_OE = 1,     /* out_odd  = H in_even, out_even = 0 */
+    CLOVER_OP_HOP_FULL = 2,   /* out = H in */
+    CLOVER_OP_CLOVER = 3,     /* out = A in */
+    CLOVER_OP_CLOVER_INV = 4, /* out = A^-1 in */
+    CLOVER_OP_D_FULL = 5,     /* out = (A - kappa H) in */
+    CLOVER_OP_MHAT = 6        /* out_even = (A_ee - kappa^2 H_eo A_oo^-1 H_oe) in_even, out_odd = 0 (R13) */
+};
+
+/* Build a context: reorder the links into the even-odd site-blocked layout (fp64 and fp32 copies,
+ * fp32 optionally two-row compressed), build the clover term A(x) from the four-leaf Fhat (S 8(c) O3),
+ * pack it as two 6x6 Hermitian blocks per site, invert the blocks (S 8(a) S0, S1).
+ * gauge_dev: canonical links (device).  Synchronises `stream` before returning. */
+int clover_create(clover_ctx **out, const double *gauge_dev, const int dims[4], double kappa, double c_sw,
+                  const int bc[4], const clover_opts *opts, void *stream);
+void clover_destroy(clover_ctx *ctx);
+
+/* out = op(in) for n_rhs spinors in canonical layout (device), precision = 32 | 64 selects both the
+ * arithmetic and the element type of in/out.  Asynchronous on `stream`.  in and out must not alias. */
+int dslash_apply(clover_ctx *ctx, int op, int precision, const void *in_dev, void *out_dev, int n_rhs, void *stream);
+
+/* Solve D psi_r = eta_r, r = 0..n_rhs-1, canonical fp64 in and out (device), by even-odd
+ * preconditioned BiCGStab batched `batch` right-hand sides per Dslash launch (1, 2, 4 or 8, <= max_rhs):
+ * mixed = 1: fp32 iteration with fp64 reliable updates (S 8(c) O6'); mixed = 0: everything fp64.
+ * Stops when the fp64 residual ||eta - D psi|| / ||eta|| <= tol (R10).  info_host: n_rhs entries, host.
+ * Synchronises `stream`.  Returns the number of non-converged sources (0 = all good) or CLOVER_E*. */
+int clover_solve(clover_ctx *ctx, const double *sources_dev, double *propagators_dev, int n_rhs, double tol,
+                 int max_iter, int batch, int mixed, clover_rhs_info *info_host, void *stream);
+
+/* Same, end to end from HOST buffers: each batch is copied host -> device, solved, and its
+ * propagators copied device -> host, all on `stream` (used for the e2e measurement). */
+int clover_solve_host(clover_ctx *ctx, const double *sources_host, double *propagators_host, int n_rhs, double tol,
+                      int max_iter, int batch, int mixed, clover_rhs_info *info_host, void *stream);
+
+/* Z4 noise sources (docs/NOISE.md): out_dev = n_rhs canonical spinors, precision 32 | 64,
+ * source index r = rhs_offset + j; time_dilution = 1 keeps only timeslice t = r mod T.
+ * Needs no context.  Asynchronous on `stream`.  Bit-exact against the written spec. */
+int noise_fill(void *out_dev, int precision, const int dims[4], uint64_t seed, int n_rhs, int rhs_offset,
+               int time_dilution, double scale, void *stream);
+
+/* ---- measurement helpers (internal layout, no reorders; used by bench.py and the ncu runs) ---- */
+enum {
+    CLOVER_KERNEL_HOP = 0,        /* out_e = H_eo in_o                          (1320 flop/site)  */
+    CLOVER_KERNEL_AINV_HOP = 1,   /* t_o = A_oo^-1 H_oe x_e                      (1824 flop/site) */
+    CLOVER_KERNEL_A_MINUS_HOP = 2 /* y_e = A_ee x_e - kappa^2 H_eo t_o + dots    (1872 flop/site) */
+};
+/* Launch one Dslash-type kernel `reps` times back to back on internal-layout scratch fields filled with
+ * pseudo-random data and return the mean device time per launch in milliseconds (CUDA events on
+ * `stream`).  precision 32 | 64; n_rhs in {1,2,4,8}.  flush_l2 != 0 writes a 256 MB buffer between
+ * launches (outside the event pairs). */
+int clover_bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms_per_launch,
+                        void *stream);
+
+/* Counters of the last clover_solve* call on this context: kernels launched, and device time (ms) spent
+ * in the phases {reorder in/out, source prep, iteration, reliable updates, reconstruct+verify}. */
+typedef struct {
+    long long kernel_launches;
+    double ms_total, ms_reorder, ms_prep, ms_iterate, ms_reliable, ms_finish;
+} clover_solve_stats;
+int clover_get_stats(const clover_ctx *ctx, clover_solve_stats *out);
+
+/* Message for the last error on the calling thread (never NULL; ctx may be NULL). */
+const char *clover_last_error(const clover_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

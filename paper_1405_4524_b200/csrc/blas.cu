@@ -1,0 +1,380 @@
+// blas.cu -- fused BLAS-1 updates, deterministic two-stage reductions and the per-rhs scalar recurrences of the
+// batched BiCGStab (SURVEY 8(a) H5, 8(c) O6').  Fields are lane-blocked (common.cuh): vector i of a field belongs
+// to rhs = i & (B-1), so every kernel is a flat, fully coalesced sweep over 16-byte vectors.
+// Reductions: products in the storage precision, accumulation in fp64, warp shuffle -> shared memory ->
+// per-block partials [block][rhs][4]; the scalar kernels sum the partials in a fixed order (deterministic).
+#include "blas.cuh"
+#include <algorithm>
+
+namespace clv {
+
+constexpr int BLAS_BLOCK = 256;
+constexpr int BLAS_MAX_GRID = 148 * 8;
+
+// ---- complex helpers on 16-byte vectors -----------------------------------------------------------
+struct zs {
+    double re, im;
+};  // a complex scalar
+__device__ __forceinline__ zs ld_z(const double2 &v) { return zs{v.x, v.y}; }
+
+// a + z*b  (per complex component of the vector)
+__device__ __forceinline__ float4 caxpy(zs z, float4 b, float4 a)
+{
+    const float zr = (float)z.re, zi = (float)z.im;
+    a.x += zr * b.x - zi * b.y;
+    a.y += zr * b.y + zi * b.x;
+    a.z += zr * b.z - zi * b.w;
+    a.w += zr * b.w + zi * b.z;
+    return a;
+}
+__device__ __forceinline__ double2 caxpy(zs z, double2 b, double2 a)
+{
+    a.x += z.re * b.x - z.im * b.y;
+    a.y += z.re * b.y + z.im * b.x;
+    return a;
+}
+__device__ __forceinline__ zs neg(zs z) { return zs{-z.re, -z.im}; }
+// conj(a) . b accumulated in fp64, |a|^2
+__device__ __forceinline__ void cdot_acc(float4 a, float4 b, double &re, double &im)
+{
+    re += (double)(a.x * b.x + a.y * b.y + a.z * b.z + a.w * b.w);
+    im += (double)(a.x * b.y - a.y * b.x + a.z * b.w - a.w * b.z);
+}
+__device__ __forceinline__ void cdot_acc(double2 a, double2 b, double &re, double &im)
+{
+    re += a.x * b.x + a.y * b.y;
+    im += a.x * b.y - a.y * b.x;
+}
+__device__ __forceinline__ double norm2(float4 a) { return (double)(a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w); }
+__device__ __forceinline__ double norm2(double2 a) { return a.x * a.x + a.y * a.y; }
+
+// block reduction with runtime B (B | 32); partial[(block*B + rhs)*4 + c]
+__device__ __forceinline__ void block_reduce(int B, double v0, double v1, double v2, double *__restrict__ partial)
+{
+    __shared__ double sm[BLAS_BLOCK / 32][8][3];
+    for (int off = 16; off >= B; off >>= 1) {
+        v0 += __shfl_xor_sync(0xffffffffu, v0, off);
+        v1 += __shfl_xor_sync(0xffffffffu, v1, off);
+        v2 += __shfl_xor_sync(0xffffffffu, v2, off);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane < B) {
+        sm[warp][lane][0] = v0;
+        sm[warp][lane][1] = v1;
+        sm[warp][lane][2] = v2;
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < B * 3) {
+        const int r = threadIdx.x / 3, c = threadIdx.x % 3;
+        double s = 0;
+        for (int w = 0; w < BLAS_BLOCK / 32; w++) s += sm[w][r][c];
+        partial[((size_t)blockIdx.x * B + r) * 4 + c] = s;
+    }
+}
+
+static inline int blas_grid(size_t nvec) { return (int)std::min<size_t>((nvec + BLAS_BLOCK - 1) / BLAS_BLOCK, BLAS_MAX_GRID); }
+
+// ---- s = r - alpha v --------------------------------------------------------------------------------
+template <typename V> __global__ void __launch_bounds__(BLAS_BLOCK) s_update_kernel(size_t n, int B, const RhsScalars *__restrict__ sc,
+                                                                                     const V *__restrict__ r, const V *__restrict__ v, V *__restrict__ s)
+{
+    const zs ma = neg(ld_z(sc[threadIdx.x & (B - 1)].alpha));
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) s[i] = caxpy(ma, v[i], r[i]);
+}
+
+// ---- x += alpha p + omega s ; r = s - omega t ; <r0,r>, ||r||^2 ----------------------------------------
+template <typename V>
+__global__ void __launch_bounds__(BLAS_BLOCK) xr_update_kernel(size_t n, int B, const RhsScalars *__restrict__ sc, V *__restrict__ x, V *__restrict__ r,
+                                                               const V *__restrict__ p, const V *__restrict__ s, const V *__restrict__ t,
+                                                               const V *__restrict__ r0, double *__restrict__ partial)
+{
+    const RhsScalars &q = sc[threadIdx.x & (B - 1)];
+    const zs al = ld_z(q.alpha), om = ld_z(q.omega), mom = neg(om);
+    double d0 = 0, d1 = 0, d2 = 0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        const V sv = s[i];
+        x[i] = caxpy(om, sv, caxpy(al, p[i], x[i]));
+        const V rn = caxpy(mom, t[i], sv);
+        r[i] = rn;
+        cdot_acc(r0[i], rn, d0, d1);
+        d2 += norm2(rn);
+    }
+    block_reduce(B, d0, d1, d2, partial);
+}
+
+// ---- p = r + beta (p - omega v) ---------------------------------------------------------------------
+template <typename V> __global__ void __launch_bounds__(BLAS_BLOCK) p_update_kernel(size_t n, int B, const RhsScalars *__restrict__ sc, V *__restrict__ p,
+                                                                                     const V *__restrict__ r, const V *__restrict__ v)
+{
+    const RhsScalars &q = sc[threadIdx.x & (B - 1)];
+    const zs be = ld_z(q.beta), mom = neg(ld_z(q.omega));
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) p[i] = caxpy(be, caxpy(mom, v[i], p[i]), r[i]);
+}
+
+// ---- y += x ; x = 0.  fp32 x: vector (jb, k, lane) holds the complex numbers 2k, 2k+1 = fp64 vectors (jb, 2k), (jb, 2k+1) ----
+__global__ void __launch_bounds__(BLAS_BLOCK) accumulate_y_kernel(size_t n32, double2 *__restrict__ y, float4 *__restrict__ x)
+{
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n32; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        const size_t lane = i & 31, row = i >> 5;  // row = jb*6 + k
+        const size_t jb = row / 6, k = row % 6;
+        const size_t o = ((jb * 12 + 2 * k) << 5) + lane;
+        const float4 v = x[i];
+        double2 a = y[o], b = y[o + 32];
+        a.x += (double)v.x; a.y += (double)v.y;
+        b.x += (double)v.z; b.y += (double)v.w;
+        y[o] = a;
+        y[o + 32] = b;
+        x[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+__global__ void __launch_bounds__(BLAS_BLOCK) accumulate_y_kernel(size_t n64, double2 *__restrict__ y, double2 *__restrict__ x)
+{
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n64; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        double2 a = y[i];
+        const double2 v = x[i];
+        a.x += v.x; a.y += v.y;
+        y[i] = a;
+        x[i] = make_double2(0., 0.);
+    }
+}
+
+// ---- r64 = b - w ; rs = (R) r64 ; ||r64||^2.  Indexed by the fp64 vector index. -------------------------
+__device__ __forceinline__ void store_sloppy(float4 *rs, size_t i, double2 v)
+{
+    // fp64 vector (jb, kk, lane) -> half of fp32 vector (jb, kk/2, lane)
+    const size_t lane = i & 31, row = i >> 5, jb = row / 12, kk = row % 12;
+    float2 *dst = reinterpret_cast<float2 *>(rs + (((jb * 6 + (kk >> 1)) << 5) + lane)) + (kk & 1);
+    *dst = make_float2((float)v.x, (float)v.y);
+}
+__device__ __forceinline__ void store_sloppy(double2 *rs, size_t i, double2 v) { rs[i] = v; }
+
+template <typename V>
+__global__ void __launch_bounds__(BLAS_BLOCK) residual_kernel(size_t n64, int B, const double2 *__restrict__ b, const double2 *__restrict__ w,
+                                                              double2 *__restrict__ r64, V *__restrict__ rs, double *__restrict__ partial)
+{
+    double d0 = 0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n64; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        double2 v = b[i];
+        if (w) {
+            const double2 ww = w[i];
+            v.x -= ww.x;
+            v.y -= ww.y;
+        }
+        r64[i] = v;
+        store_sloppy(rs, i, v);
+        d0 += norm2(v);
+    }
+    block_reduce(B, d0, 0., 0., partial);
+}
+
+// ---- d0 = ||a1 - b1||^2, d1 = ||a2 - b2||^2 (b1, b2 may be null) --------------------------------------------
+__device__ __forceinline__ double diff2(const double2 *__restrict__ a, const double2 *__restrict__ b, size_t i)
+{
+    double2 v = a[i];
+    if (b) {
+        const double2 bb = b[i];
+        v.x -= bb.x;
+        v.y -= bb.y;
+    }
+    return norm2(v);
+}
+__global__ void __launch_bounds__(BLAS_BLOCK) norm2_pair_kernel(size_t n64, int B, const double2 *__restrict__ a1, const double2 *__restrict__ b1,
+                                                                const double2 *__restrict__ a2, const double2 *__restrict__ b2,
+                                                                double *__restrict__ partial)
+{
+    double d0 = 0, d1 = 0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n64; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        d0 += diff2(a1, b1, i);
+        d1 += diff2(a2, b2, i);
+    }
+    block_reduce(B, d0, d1, 0., partial);
+}
+
+// ---- scalar steps -----------------------------------------------------------------------------------------
+__device__ __forceinline__ zs zdiv(zs a, zs b)
+{
+    const double d = b.re * b.re + b.im * b.im;
+    return zs{(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
+}
+__device__ __forceinline__ zs zmul(zs a, zs b) { return zs{a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ double2 st_z(zs z) { return make_double2(z.re, z.im); }
+__device__ __forceinline__ bool finite_z(zs z) { return isfinite(z.re) && isfinite(z.im); }
+
+// one block per rhs: sum partial[(b*B + rhs)*4 + c] over b < nblocks in a fixed order, then thread 0 updates the scalars.
+__global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblocks, const double *__restrict__ partial, RhsScalars *sc, double tol2,
+                                                     double delta2)
+{
+    __shared__ double sm[256][3];
+    const int rhs = blockIdx.x;
+    double a0 = 0, a1 = 0, a2 = 0;
+    for (int b = threadIdx.x; b < nblocks; b += 256) {
+        const double *q = partial + ((size_t)b * B + rhs) * 4;
+        a0 += q[0];
+        a1 += q[1];
+        a2 += q[2];
+    }
+    sm[threadIdx.x][0] = a0;
+    sm[threadIdx.x][1] = a1;
+    sm[threadIdx.x][2] = a2;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s) {
+            sm[threadIdx.x][0] += sm[threadIdx.x + s][0];
+            sm[threadIdx.x][1] += sm[threadIdx.x + s][1];
+            sm[threadIdx.x][2] += sm[threadIdx.x + s][2];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x != 0) return;
+    const double d0 = sm[0][0], d1 = sm[0][1], d2 = sm[0][2];
+    RhsScalars &q = sc[rhs];
+    const zs zero{0., 0.};
+    switch (step) {
+    case SC_ETA2:  // d0 = ||eta_e||^2, d1 = ||eta_o||^2
+        q.eta2 = d0 + d1;
+        q.done = 0;
+        q.status = 0;
+        q.want_update = 0;
+        break;
+    case SC_INIT:  // d0 = ||r||^2 with r = b_e (y = 0)
+        q.rho = make_double2(d0, 0.);
+        q.r2 = q.maxr2 = q.true_r2 = d0;
+        q.alpha = q.omega = q.beta = make_double2(0., 0.);
+        q.want_update = 0;
+        if (!(q.eta2 > 0.) || d0 <= tol2 * q.eta2) q.done = 1;  // zero source or already converged
+        if (!isfinite(d0)) { q.done = 1; q.status = 3; }
+        break;
+    case SC_ALPHA: {  // (d0,d1) = <r0, v>
+        zs al = zero;
+        if (!q.done) {
+            const zs r0v{d0, d1};
+            if (!finite_z(r0v)) { q.done = 1; q.status = 3; }
+            else if (!(d0 * d0 + d1 * d1 > 0.)) { q.done = 1; q.status = 2; }
+            else al = zdiv(ld_z(q.rho), r0v);
+        }
+        q.alpha = st_z(al);
+        break;
+    }
+    case SC_OMEGA: {  // (d0,d1) = <t, s>, d2 = <t, t>
+        zs om = zero;
+        if (!q.done) {
+            if (!isfinite(d2) || !isfinite(d0) || !isfinite(d1)) { q.done = 1; q.status = 3; q.alpha = st_z(zero); }
+            else if (d2 > 0.) om = zs{d0 / d2, d1 / d2};
+        }
+        q.omega = st_z(om);
+        break;
+    }
+    case SC_RHO: {  // (d0,d1) = <r0, r>, d2 = ||r||^2
+        zs be = zero;
+        q.want_update = 0;
+        if (!q.done) {
+            const zs rho1{d0, d1}, om = ld_z(q.omega), rho = ld_z(q.rho);
+            q.r2 = d2;
+            if (d2 > q.maxr2) q.maxr2 = d2;
+            if (!isfinite(d2) || !finite_z(rho1)) { q.done = 1; q.status = 3; }
+            else {
+                if (d2 < delta2 * q.maxr2 || d2 <= tol2 * q.eta2) q.want_update = 1;
+                const double om2 = om.re * om.re + om.im * om.im, rh2 = rho.re * rho.re + rho.im * rho.im;
+                if (!(om2 > 0.) || !(rh2 > 0.)) q.want_update = 1;  // stagnation: let the fp64 residual decide, beta = 0 restarts p = r
+                else be = zmul(zdiv(rho1, rho), zdiv(ld_z(q.alpha), om));
+                if (!finite_z(be)) be = zero;
+                q.rho = st_z(rho1);
+            }
+        }
+        q.beta = st_z(be);
+        break;
+    }
+    case SC_TRUE:  // d0 = ||b - Mhat y||^2 in fp64
+        q.true_r2 = d0;
+        if (!q.done) {
+            q.r2 = q.maxr2 = d0;
+            q.want_update = 0;
+            if (!isfinite(d0)) { q.done = 1; q.status = 3; }
+            else if (d0 <= tol2 * q.eta2) { q.done = 1; q.beta = st_z(zero); }
+        }
+        break;
+    case SC_FINAL:  // d0 + d1 = ||eta - D psi||^2 on the full lattice; stored in r2 (true_r2 keeps the even-odd value)
+        q.r2 = d0 + d1;
+        break;
+    }
+}
+
+// ---- host wrappers ---------------------------------------------------------------------------------------
+#define BLAS_LAUNCHED(c) do { if ((c).launches) ++*(c).launches; } while (0)
+
+template <typename R> int blas_s_update(const BlasCtx &c, const typename Vec<R>::T *r, const typename Vec<R>::T *v, typename Vec<R>::T *s)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    s_update_kernel<<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, r, v, s);
+    BLAS_LAUNCHED(c);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R>
+int blas_xr_update(const BlasCtx &c, typename Vec<R>::T *x, typename Vec<R>::T *r, const typename Vec<R>::T *p, const typename Vec<R>::T *s,
+                   const typename Vec<R>::T *t, const typename Vec<R>::T *r0, int *nblocks)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    const int grid = blas_grid(n);
+    xr_update_kernel<<<grid, BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, x, r, p, s, t, r0, c.partial);
+    BLAS_LAUNCHED(c);
+    *nblocks = grid;
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R> int blas_p_update(const BlasCtx &c, typename Vec<R>::T *p, const typename Vec<R>::T *r, const typename Vec<R>::T *v)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    p_update_kernel<<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, p, r, v);
+    BLAS_LAUNCHED(c);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R> int blas_accumulate_y(const BlasCtx &c, double2 *y, typename Vec<R>::T *x)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    accumulate_y_kernel<<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, y, x);
+    BLAS_LAUNCHED(c);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R> int blas_residual(const BlasCtx &c, const double2 *b, const double2 *w, double2 *r64, typename Vec<R>::T *rs, int *nblocks)
+{
+    const size_t n = field_vecs<double>(*c.g, c.B);
+    const int grid = blas_grid(n);
+    residual_kernel<<<grid, BLAS_BLOCK, 0, c.st>>>(n, c.B, b, w, r64, rs, c.partial);
+    BLAS_LAUNCHED(c);
+    *nblocks = grid;
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, const double2 *a2, const double2 *b2, int *nblocks)
+{
+    const size_t n = field_vecs<double>(*c.g, c.B);
+    const int grid = blas_grid(n);
+    norm2_pair_kernel<<<grid, BLAS_BLOCK, 0, c.st>>>(n, c.B, a1, b1, a2, b2, c.partial);
+    BLAS_LAUNCHED(c);
+    *nblocks = grid;
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2)
+{
+    scalar_kernel<<<c.B, 256, 0, c.st>>>(step, c.B, nblocks, c.partial, c.sc, tol2, delta2);
+    BLAS_LAUNCHED(c);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+
+#define INST(R)                                                                                                                                  \
+    template int blas_s_update<R>(const BlasCtx &, const Vec<R>::T *, const Vec<R>::T *, Vec<R>::T *);                                           \
+    template int blas_xr_update<R>(const BlasCtx &, Vec<R>::T *, Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *,          \
+                                   const Vec<R>::T *, int *);                                                                                    \
+    template int blas_p_update<R>(const BlasCtx &, Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *);                                           \
+    template int blas_accumulate_y<R>(const BlasCtx &, double2 *, Vec<R>::T *);                                                                  \
+    template int blas_residual<R>(const BlasCtx &, const double2 *, const double2 *, double2 *, Vec<R>::T *, int *);
+INST(float)
+INST(double)
+#undef INST
+
+}  // namespace clv

@@ -1,0 +1,39 @@
+// blas.cuh -- host interface of the fused BLAS-1 / reduction / scalar kernels of the batched BiCGStab.
+#pragma once
+#include "context.h"
+
+namespace clv {
+
+// number of 16-byte vectors of a half-lattice field with B rhs
+template <typename R> inline size_t field_vecs(const Geom &g, int B) { return (size_t)lb_blocks((unsigned)g.Vh * B) * 32u * Vec<R>::NV; }
+
+struct BlasCtx {
+    const Geom *g;
+    int B;
+    RhsScalars *sc;    // device, B entries
+    double *partial;   // device, [blocks][B][4]
+    int max_partial_blocks;
+    cudaStream_t st;
+    long long *launches;
+};
+
+// s = r - alpha v
+template <typename R> int blas_s_update(const BlasCtx &c, const typename Vec<R>::T *r, const typename Vec<R>::T *v, typename Vec<R>::T *s);
+// x += alpha p + omega s ; r = s - omega t ; partial <r0,r>, ||r||^2 ; returns number of partial blocks
+template <typename R>
+int blas_xr_update(const BlasCtx &c, typename Vec<R>::T *x, typename Vec<R>::T *r, const typename Vec<R>::T *p, const typename Vec<R>::T *s,
+                   const typename Vec<R>::T *t, const typename Vec<R>::T *r0, int *nblocks);
+// p = r + beta (p - omega v)
+template <typename R> int blas_p_update(const BlasCtx &c, typename Vec<R>::T *p, const typename Vec<R>::T *r, const typename Vec<R>::T *v);
+// y += x (fp64 accumulate), x = 0
+template <typename R> int blas_accumulate_y(const BlasCtx &c, double2 *y, typename Vec<R>::T *x);
+// r64 = b - w (w may be null: r64 = b) ; rs = (R) r64 ; partial ||r64||^2
+template <typename R> int blas_residual(const BlasCtx &c, const double2 *b, const double2 *w, double2 *r64, typename Vec<R>::T *rs, int *nblocks);
+// partial d0 = ||a1 - b1||^2, d1 = ||a2 - b2||^2 (b1, b2 may be null)
+int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, const double2 *a2, const double2 *b2, int *nblocks);
+
+// scalar steps (one block per rhs): reduce the partials of `nblocks` blocks and update RhsScalars
+enum { SC_ETA2 = 0, SC_INIT = 1, SC_ALPHA = 2, SC_OMEGA = 3, SC_RHO = 4, SC_TRUE = 5, SC_FINAL = 6 };
+int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2);
+
+}  // namespace clv

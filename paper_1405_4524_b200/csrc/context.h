@@ -1,0 +1,91 @@
+// context.h -- the opaque clover_ctx and the internal (host-side) interfaces between translation units.
+#pragma once
+#include "../../include/clover.h"
+#include "common.cuh"
+#include <vector>
+
+namespace clv {
+
+// Per-precision operator data in the internal layout (device pointers owned by the context).
+template <typename R> struct OpData {
+    typedef typename Vec<R>::C C;
+    C *gauge[2][4];   // [parity of the site the link lives at][mu], lane-blocked over cb, NK = recon/2
+    C *clov[2];       // A   : [parity], 36 complex per site (2 blocks x (3 packed diag pairs + 15 lower off-diag))
+    C *clov_inv[2];   // A^-1, same packing
+    int recon;        // 18 | 12
+};
+
+// Per-rhs solver scalars, device resident (one entry per rhs of the batch).
+struct RhsScalars {
+    double2 rho, alpha, omega, beta;  // BiCGStab recurrences (complex)
+    double r2;        // ||r||^2 of the iterated (sloppy) residual
+    double maxr2;     // max ||r||^2 since the last reliable update
+    double eta2;      // ||eta||^2 on the full lattice (stopping scale, R10)
+    double true_r2;   // ||r||^2 at the last fp64 recomputation
+    int done;         // 1 once the fp64 residual met the tolerance (rhs frozen)
+    int want_update;  // 1 if this rhs asks for a reliable update
+    int status;       // clover_rhs_info.status
+    int pad;
+};
+
+struct SolveWork;  // solver.cu
+
+}  // namespace clv
+
+struct clover_ctx {
+    clv::Geom geom;
+    double kappa, csw;
+    int max_rhs;
+    clv::OpData<double> op64;
+    clv::OpData<float> op32;
+    // scratch fields (internal layout) sized for max_rhs, allocated lazily by the solver / bench / dslash_apply
+    clv::SolveWork *work;
+    clover_solve_stats stats;
+    std::vector<void *> allocs;  // every device allocation of the operator data (freed by clover_destroy)
+};
+
+namespace clv {
+
+// ---- setup.cu ----
+int setup_operator(clover_ctx *ctx, const double *gauge_dev, cudaStream_t st);
+// canonical <-> internal reorders; CT = element type of the canonical array, R = internal real type.
+// canon: [n_rhs][V][12] complex of CT; even/odd: internal fields with B = n_rhs.
+template <typename CT, typename R>
+int reorder_in(const Geom &g, const CT *canon, typename Vec<R>::T *even, typename Vec<R>::T *odd, int B, cudaStream_t st);
+template <typename CT, typename R>
+int reorder_out(const Geom &g, CT *canon, const typename Vec<R>::T *even, const typename Vec<R>::T *odd, int B, cudaStream_t st);
+
+// ---- dslash.cu ----
+// out = P ( X + coef * H_{p,1-p} in ),  P = 1 | A_pp^-1,  X = 0 | xin | A_pp xin   (p = parity of out)
+enum { XM_NONE = 0, XM_PLAIN = 1, XM_CLOVER = 2 };
+enum { DOT_NONE = 0, DOT_W = 1, DOT_X = 2 };
+template <typename R> struct DslashArgs {
+    typedef typename Vec<R>::T V;
+    const V *in;      // parity 1-p field
+    const V *xin;     // parity p field (XM_PLAIN / XM_CLOVER)
+    V *out;           // parity p field
+    const V *w;       // DOT_W: partial <w, out> per rhs
+    double *partial;  // [gridDim.x][B][4] : DOT_W -> (re,im of <w,out>, 0, 0); DOT_X -> (re,im of <out,xin>, <out,out>, 0)
+    R coef;
+    int parity;       // p
+    int xmode, pinv, dot;
+};
+template <typename R> int launch_dslash(const clover_ctx *ctx, const DslashArgs<R> &a, int B, cudaStream_t st, int *grid_out);
+// out = A in or A^-1 in on one parity
+template <typename R>
+int launch_clover(const clover_ctx *ctx, const typename Vec<R>::T *in, typename Vec<R>::T *out, int parity, int inverse, int B,
+                  cudaStream_t st);
+int dslash_block_size();
+
+// ---- noise.cu ----
+int launch_noise(void *out, int precision, const int dims[4], uint64_t seed, int n_rhs, int rhs_offset, int dilution, double scale,
+                 cudaStream_t st);
+
+// ---- solver.cu ----
+int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, double tol, int max_iter, int batch, int mixed,
+                  clover_rhs_info *info, cudaStream_t st, int host_buffers);
+void free_work(clover_ctx *ctx);
+int bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms, cudaStream_t st);
+int apply_op(clover_ctx *ctx, int op, int precision, const void *in, void *out, int n_rhs, cudaStream_t st);
+
+}  // namespace clv

@@ -1,0 +1,63 @@
+// dslash_inst.cuh -- host dispatch of one (precision, batch) family of Dslash kernels; included by the
+// dslash_<prec>_b<B>.cu instantiation units so the variants compile in parallel.
+#pragma once
+#include "dslash_kernel.cuh"
+
+namespace clv {
+
+template <typename R, int B, int RECON>
+static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const DslashArgs<R> &a, cudaStream_t st, int *grid_out)
+{
+    const Geom &g = ctx->geom;
+    const unsigned n = (unsigned)g.Vh * B;
+    const unsigned grid = (n + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
+    if (grid_out) *grid_out = (int)grid;
+    const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
+#define CLV_LAUNCH(XM, PI, DT)                                                          \
+    case (XM) * 100 + (PI) * 10 + (DT):                                                 \
+        dslash_kernel<R, B, RECON, XM, PI, DT><<<grid, DSLASH_BLOCK, 0, st>>>(g, op, a); \
+        break;
+    switch (key) {
+        CLV_LAUNCH(XM_NONE, 0, DOT_NONE)
+        CLV_LAUNCH(XM_NONE, 1, DOT_NONE)
+        CLV_LAUNCH(XM_PLAIN, 0, DOT_NONE)
+        CLV_LAUNCH(XM_PLAIN, 1, DOT_NONE)
+        CLV_LAUNCH(XM_CLOVER, 0, DOT_NONE)
+        CLV_LAUNCH(XM_CLOVER, 0, DOT_W)
+        CLV_LAUNCH(XM_CLOVER, 0, DOT_X)
+    default:
+        set_error("dslash: unsupported variant xmode=%d pinv=%d dot=%d", a.xmode, a.pinv, a.dot);
+        return CLOVER_EINVAL;
+    }
+#undef CLV_LAUNCH
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+
+template <typename R> struct OpSel;
+template <> struct OpSel<float> { static const OpData<float> &get(const clover_ctx *c) { return c->op32; } };
+template <> struct OpSel<double> { static const OpData<double> &get(const clover_ctx *c) { return c->op64; } };
+
+template <typename R, int B> int launch_dslash_B(const clover_ctx *ctx, const DslashArgs<R> &a, cudaStream_t st, int *grid_out)
+{
+    const OpData<R> &op = OpSel<R>::get(ctx);
+    if (op.recon == 12) {
+        if (sizeof(R) == 4) return launch_dslash_BR<R, B, (sizeof(R) == 4 ? 12 : 18)>(ctx, op, a, st, grid_out);
+        set_error("dslash: two-row links exist in fp32 only");
+        return CLOVER_EINVAL;
+    }
+    return launch_dslash_BR<R, B, 18>(ctx, op, a, st, grid_out);
+}
+
+template <typename R, int B>
+int launch_clover_B(const clover_ctx *ctx, const typename Vec<R>::T *in, typename Vec<R>::T *out, int parity, int inverse, cudaStream_t st)
+{
+    const Geom &g = ctx->geom;
+    const OpData<R> &op = OpSel<R>::get(ctx);
+    const unsigned n = (unsigned)g.Vh * B;
+    clover_kernel<R, B><<<(n + DSLASH_BLOCK - 1) / DSLASH_BLOCK, DSLASH_BLOCK, 0, st>>>(g, inverse ? op.clov_inv[parity] : op.clov[parity], in, out);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+
+}  // namespace clv

@@ -1,0 +1,420 @@
+// solver.cu -- host driver of the batched, even-odd preconditioned, mixed-precision BiCGStab (
+// 8(c) O6'): B independent recurrences share every operator application; all scalars stay on the device, the host
+// only reads back the per-rhs flags once per iteration.
+//   Mhat = A_ee - kappa^2 H_eo A_oo^-1 H_oe   on the even sites            (R13)
+//   b_e  = eta_e + kappa H_eo A_oo^-1 eta_o ;  psi_o = A_oo^-1 (eta_o + kappa H_oe psi_e)
+// Also: dslash_apply's operator table and the kernel benchmark entry.
+#include "blas.cuh"
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+
+namespace clv {
+
+struct SolveWork {
+    int B_cap = 0;
+    size_t sloppy_bytes = 0;   // bytes of each sloppy field currently allocated
+    double2 *f64[8] = {};      // eta_e, eta_o, b, y, r64, w64, tmp64, psi_o
+    void *sl[8] = {};          // x, r, p, v, s, t, r0, tmp  (float4 or double2 fields)
+    double *partial = nullptr;
+    int partial_blocks = 0;
+    RhsScalars *sc_dev = nullptr, *sc_host = nullptr;
+    double *stage_in = nullptr, *stage_out = nullptr;  // canonical staging for host-buffer solves
+    size_t stage_bytes = 0;
+    void *flush = nullptr;
+    cudaEvent_t ev[6] = {};
+    bool have_ev = false;
+};
+
+enum { F_ETA_E = 0, F_ETA_O, F_B, F_Y, F_R64, F_W64, F_TMP64, F_PSI_O };
+enum { S_X = 0, S_R, S_P, S_V, S_S, S_T, S_R0, S_TMP };
+
+void free_work(clover_ctx *ctx)
+{
+    SolveWork *W = ctx->work;
+    if (!W) return;
+    for (int i = 0; i < 8; i++) { cudaFree(W->f64[i]); cudaFree(W->sl[i]); }
+    cudaFree(W->partial);
+    cudaFree(W->sc_dev);
+    cudaFreeHost(W->sc_host);
+    cudaFree(W->stage_in);
+    cudaFree(W->stage_out);
+    cudaFree(W->flush);
+    if (W->have_ev) for (int i = 0; i < 6; i++) cudaEventDestroy(W->ev[i]);
+    delete W;
+    ctx->work = nullptr;
+}
+
+static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
+{
+    if (!ctx->work) ctx->work = new SolveWork();
+    SolveWork *W = ctx->work;
+    const Geom &g = ctx->geom;
+    if (B > W->B_cap) {
+        const size_t n64 = field_vecs<double>(g, B);
+        for (int i = 0; i < 8; i++) {
+            cudaFree(W->f64[i]);
+            W->f64[i] = nullptr;
+            CLV_CUDA(cudaMalloc(&W->f64[i], n64 * sizeof(double2)));
+            CLV_CUDA(cudaMemset(W->f64[i], 0, n64 * sizeof(double2)));
+        }
+        cudaFree(W->partial);
+        W->partial_blocks = std::max<int>(((unsigned)g.Vh * B + dslash_block_size() - 1) / dslash_block_size(), 148 * 8);
+        CLV_CUDA(cudaMalloc(&W->partial, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
+        CLV_CUDA(cudaMemset(W->partial, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
+        if (!W->sc_dev) {
+            CLV_CUDA(cudaMalloc(&W->sc_dev, 8 * sizeof(RhsScalars)));
+            CLV_CUDA(cudaMemset(W->sc_dev, 0, 8 * sizeof(RhsScalars)));
+            CLV_CUDA(cudaMallocHost(&W->sc_host, 8 * sizeof(RhsScalars)));
+        }
+        W->B_cap = B;
+        W->sloppy_bytes = 0;
+    }
+    const size_t need = field_vecs<double>(g, W->B_cap) * 16 / 8 * real_bytes;  // float fields are half the size of double ones
+    if (need > W->sloppy_bytes) {
+        for (int i = 0; i < 8; i++) {
+            cudaFree(W->sl[i]);
+            W->sl[i] = nullptr;
+            CLV_CUDA(cudaMalloc(&W->sl[i], need));
+            CLV_CUDA(cudaMemset(W->sl[i], 0, need));
+        }
+        W->sloppy_bytes = need;
+    }
+    if (staging) {
+        const size_t sb = (size_t)2 * g.Vh * 24 * sizeof(double) * W->B_cap;
+        if (sb > W->stage_bytes) {
+            cudaFree(W->stage_in);
+            cudaFree(W->stage_out);
+            W->stage_in = W->stage_out = nullptr;
+            CLV_CUDA(cudaMalloc(&W->stage_in, sb));
+            CLV_CUDA(cudaMalloc(&W->stage_out, sb));
+            W->stage_bytes = sb;
+        }
+    }
+    if (!W->have_ev) {
+        for (int i = 0; i < 6; i++) CLV_CUDA(cudaEventCreate(&W->ev[i]));
+        W->have_ev = true;
+    }
+    CLV_CUDA(cudaDeviceSynchronize());  // the memsets above ran on the legacy stream
+    return 0;
+}
+
+// Padding lanes (j >= Vh*B in the last 32-lane block) must hold zeros because the BLAS sweeps and their reductions
+// run over whole blocks.  Only lattices with Vh*B not a multiple of 32 have any; there the fields are cleared
+// whenever the batch size (hence the meaning of a lane) changes.
+static int clear_fields(SolveWork *W, const Geom &g, int B, cudaStream_t st)
+{
+    if (((unsigned)g.Vh * B) % 32u == 0) return 0;
+    const size_t n64 = field_vecs<double>(g, W->B_cap) * sizeof(double2);
+    for (int i = 0; i < 8; i++) {
+        CLV_CUDA(cudaMemsetAsync(W->f64[i], 0, n64, st));
+        CLV_CUDA(cudaMemsetAsync(W->sl[i], 0, W->sloppy_bytes, st));
+    }
+    return 0;
+}
+
+template <typename R> static DslashArgs<R> dargs(const typename Vec<R>::T *in, const typename Vec<R>::T *xin, typename Vec<R>::T *out, R coef, int parity,
+                                                int xmode, int pinv, int dot = DOT_NONE, const typename Vec<R>::T *w = nullptr, double *partial = nullptr)
+{
+    DslashArgs<R> a;
+    a.in = in; a.xin = xin; a.out = out; a.w = w; a.partial = partial; a.coef = coef; a.parity = parity;
+    a.xmode = xmode; a.pinv = pinv; a.dot = dot;
+    return a;
+}
+
+// out_e = Mhat in_e, optional fused dot products; tmp is an odd-parity scratch field
+template <typename R>
+static int mhat(clover_ctx *ctx, int B, const typename Vec<R>::T *in, typename Vec<R>::T *tmp, typename Vec<R>::T *out, int dot, const typename Vec<R>::T *w,
+                double *partial, int *grid, cudaStream_t st)
+{
+    const R k2 = (R)(-ctx->kappa * ctx->kappa);
+    CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(in, nullptr, tmp, (R)1, 1, XM_NONE, 1), B, st, nullptr));
+    CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(tmp, in, out, k2, 0, XM_CLOVER, 0, dot, w, partial), B, st, grid));
+    ctx->stats.kernel_launches += 2;
+    return 0;
+}
+
+static int fetch_scalars(SolveWork *W, int B, cudaStream_t st)
+{
+    CLV_CUDA(cudaMemcpyAsync(W->sc_host, W->sc_dev, B * sizeof(RhsScalars), cudaMemcpyDeviceToHost, st));
+    CLV_CUDA(cudaStreamSynchronize(st));
+    return 0;
+}
+
+static double reliable_delta()
+{
+    const char *e = getenv("CLOVER_DELTA");  // tuning/debug knob only
+    const double d = e ? atof(e) : 0.0;
+    return (d > 0.0 && d < 1.0) ? d : 0.05;
+}
+
+template <typename R>
+static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, double tol, int max_iter, clover_rhs_info *info, cudaStream_t st)
+{
+    typedef typename Vec<R>::T V;
+    SolveWork *W = ctx->work;
+    const Geom &g = ctx->geom;
+    double2 *eta_e = W->f64[F_ETA_E], *eta_o = W->f64[F_ETA_O], *b = W->f64[F_B], *y = W->f64[F_Y], *r64 = W->f64[F_R64], *w64 = W->f64[F_W64],
+            *tmp64 = W->f64[F_TMP64], *psi_o = W->f64[F_PSI_O];
+    V *x = (V *)W->sl[S_X], *r = (V *)W->sl[S_R], *p = (V *)W->sl[S_P], *v = (V *)W->sl[S_V], *s = (V *)W->sl[S_S], *t = (V *)W->sl[S_T],
+      *r0 = (V *)W->sl[S_R0], *tmp = (V *)W->sl[S_TMP];
+    long long &nl = ctx->stats.kernel_launches;
+    BlasCtx bc{&g, B, W->sc_dev, W->partial, W->partial_blocks, st, &nl};
+    const double tol2 = tol * tol, delta = reliable_delta(), delta2 = delta * delta;
+    const size_t nbytes = field_vecs<R>(g, B) * sizeof(V), nbytes64 = field_vecs<double>(g, B) * sizeof(double2);
+    int nb = 0, grid = 0, iters = 0, updates = 0;
+    float ms;
+
+    CLV_CUDA(cudaEventRecord(W->ev[0], st));
+    CLV_CHECK((reorder_in<double, double>(g, src, eta_e, eta_o, B, st)));
+    nl++;
+    CLV_CUDA(cudaEventRecord(W->ev[1], st));
+    // stopping scale ||eta||^2 (R10) and source preparation b_e = eta_e + kappa H_eo A_oo^-1 eta_o
+    CLV_CHECK(blas_norm2_pair(bc, eta_e, nullptr, eta_o, nullptr, &nb));
+    CLV_CHECK(blas_scalar_step(bc, SC_ETA2, nb, tol2, delta2));
+    CLV_CHECK(launch_clover<double>(ctx, eta_o, tmp64, 1, 1, B, st));
+    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(tmp64, eta_e, b, ctx->kappa, 0, XM_PLAIN, 0), B, st, nullptr));
+    nl += 2;
+    // y = 0, x = 0, r = b, p = r0 = r
+    CLV_CUDA(cudaMemsetAsync(y, 0, nbytes64, st));
+    CLV_CUDA(cudaMemsetAsync(x, 0, nbytes, st));
+    CLV_CHECK(blas_residual<R>(bc, b, nullptr, r64, r, &nb));
+    CLV_CHECK(blas_scalar_step(bc, SC_INIT, nb, tol2, delta2));
+    CLV_CUDA(cudaMemcpyAsync(p, r, nbytes, cudaMemcpyDeviceToDevice, st));
+    CLV_CUDA(cudaMemcpyAsync(r0, r, nbytes, cudaMemcpyDeviceToDevice, st));
+    CLV_CUDA(cudaEventRecord(W->ev[2], st));
+    CLV_CHECK(fetch_scalars(W, B, st));
+
+    auto all_done = [&]() { for (int i = 0; i < B; i++) if (!W->sc_host[i].done) return false; return true; };
+    auto any_update = [&]() { for (int i = 0; i < B; i++) if (!W->sc_host[i].done && W->sc_host[i].want_update) return true; return false; };
+    double ms_reliable = 0;
+    while (!all_done() && iters < max_iter) {
+        CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_W, r0, W->partial, &grid, st));
+        CLV_CHECK(blas_scalar_step(bc, SC_ALPHA, grid, tol2, delta2));
+        CLV_CHECK(blas_s_update<R>(bc, r, v, s));
+        CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_X, nullptr, W->partial, &grid, st));
+        CLV_CHECK(blas_scalar_step(bc, SC_OMEGA, grid, tol2, delta2));
+        CLV_CHECK(blas_xr_update<R>(bc, x, r, p, s, t, r0, &nb));
+        CLV_CHECK(blas_scalar_step(bc, SC_RHO, nb, tol2, delta2));
+        CLV_CHECK(fetch_scalars(W, B, st));
+        iters++;
+        if (any_update() || iters == max_iter) {
+            // reliable update: y += x, x = 0, r = b - Mhat y in fp64 (S 8(c) O6')
+            CLV_CUDA(cudaEventRecord(W->ev[4], st));
+            CLV_CHECK(blas_accumulate_y<R>(bc, y, x));
+            CLV_CHECK(mhat<double>(ctx, B, y, tmp64, w64, DOT_NONE, nullptr, nullptr, nullptr, st));
+            CLV_CHECK(blas_residual<R>(bc, b, w64, r64, r, &nb));
+            CLV_CHECK(blas_scalar_step(bc, SC_TRUE, nb, tol2, delta2));
+            CLV_CUDA(cudaEventRecord(W->ev[5], st));
+            CLV_CHECK(fetch_scalars(W, B, st));
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[4], W->ev[5]));
+            ms_reliable += ms;
+            updates++;
+        }
+        if (all_done()) break;
+        CLV_CHECK(blas_p_update<R>(bc, p, r, v));
+    }
+    CLV_CUDA(cudaEventRecord(W->ev[3], st));
+    // odd sites and verification on the full lattice, all fp64
+    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, eta_o, psi_o, ctx->kappa, 1, XM_PLAIN, 1), B, st, nullptr));
+    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(psi_o, y, w64, -ctx->kappa, 0, XM_CLOVER, 0), B, st, nullptr));
+    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, psi_o, tmp64, -ctx->kappa, 1, XM_CLOVER, 0), B, st, nullptr));
+    nl += 3;
+    CLV_CHECK(blas_norm2_pair(bc, eta_e, w64, eta_o, tmp64, &nb));
+    CLV_CHECK(blas_scalar_step(bc, SC_FINAL, nb, tol2, delta2));
+    CLV_CUDA(cudaEventRecord(W->ev[4], st));
+    CLV_CHECK((reorder_out<double, double>(g, dst, y, psi_o, B, st)));
+    nl++;
+    CLV_CUDA(cudaEventRecord(W->ev[5], st));
+    CLV_CHECK(fetch_scalars(W, B, st));
+
+    clover_solve_stats &S = ctx->stats;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[0], W->ev[1])); S.ms_reorder += ms;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[4], W->ev[5])); S.ms_reorder += ms;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[1], W->ev[2])); S.ms_prep += ms;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[2], W->ev[3])); S.ms_iterate += ms - ms_reliable;
+    S.ms_reliable += ms_reliable;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[3], W->ev[4])); S.ms_finish += ms;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[0], W->ev[5])); S.ms_total += ms;
+
+    int bad = 0;
+    for (int i = 0; i < B; i++) {
+        const RhsScalars &q = W->sc_host[i];
+        clover_rhs_info &o = info[i];
+        o.iters = iters;
+        o.reliable_updates = updates;
+        o.iter_resid = q.eta2 > 0 ? sqrt(q.true_r2 / q.eta2) : 0.0;
+        o.true_resid = q.eta2 > 0 ? sqrt(q.r2 / q.eta2) : 0.0;
+        o.status = q.status;
+        if (o.status == 0 && !(o.true_resid <= tol)) o.status = (o.true_resid == o.true_resid) ? 1 : 3;
+        if (o.status != 0) bad++;
+    }
+    return bad;
+}
+
+// greedy split of n into batches from {8,4,2,1} not exceeding `batch`
+static int next_batch(int remaining, int batch)
+{
+    int b = 1;
+    while (b * 2 <= batch && b * 2 <= remaining) b *= 2;
+    return b;
+}
+
+int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, double tol, int max_iter, int batch, int mixed, clover_rhs_info *info,
+                  cudaStream_t st, int host_buffers)
+{
+    CLV_CHECK(ensure_work(ctx, batch, mixed ? 4 : 8, host_buffers != 0));
+    SolveWork *W = ctx->work;
+    memset(&ctx->stats, 0, sizeof ctx->stats);
+    const size_t per_rhs = (size_t)2 * ctx->geom.Vh * 24;  // doubles per canonical spinor
+    int bad = 0, lastB = -1;
+    for (int done = 0; done < n_rhs;) {
+        const int B = next_batch(n_rhs - done, batch);
+        if (B != lastB) CLV_CHECK(clear_fields(W, ctx->geom, B, st));
+        lastB = B;
+        const double *s = src + done * per_rhs;
+        double *d = dst + done * per_rhs;
+        if (host_buffers) {
+            CLV_CUDA(cudaMemcpyAsync(W->stage_in, s, per_rhs * B * sizeof(double), cudaMemcpyHostToDevice, st));
+            s = W->stage_in;
+            d = W->stage_out;
+        }
+        int rc = mixed ? solve_batch<float>(ctx, s, d, B, tol, max_iter, info + done, st) : solve_batch<double>(ctx, s, d, B, tol, max_iter, info + done, st);
+        if (rc < 0) return rc;
+        bad += rc;
+        if (host_buffers) {
+            CLV_CUDA(cudaMemcpyAsync(dst + done * per_rhs, W->stage_out, per_rhs * B * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CLV_CUDA(cudaStreamSynchronize(st));
+        }
+        done += B;
+    }
+    return bad;
+}
+
+// ---- dslash_apply: canonical in -> op -> canonical out --------------------------------------------------------
+template <typename R> struct Canon;
+template <> struct Canon<float> { typedef float T; };
+template <> struct Canon<double> { typedef double T; };
+
+template <typename R> static int apply_chunk(clover_ctx *ctx, int op, const R *in, R *out, int B, cudaStream_t st)
+{
+    typedef typename Vec<R>::T V;
+    SolveWork *W = ctx->work;
+    const Geom &g = ctx->geom;
+    V *ie, *io, *oe, *oo, *tmp;
+    if (sizeof(R) == 8) {
+        ie = (V *)W->f64[0]; io = (V *)W->f64[1]; oe = (V *)W->f64[2]; oo = (V *)W->f64[3]; tmp = (V *)W->f64[4];
+    } else {
+        ie = (V *)W->sl[0]; io = (V *)W->sl[1]; oe = (V *)W->sl[2]; oo = (V *)W->sl[3]; tmp = (V *)W->sl[4];
+    }
+    CLV_CHECK((reorder_in<R, R>(g, in, ie, io, B, st)));
+    const R one = (R)1, mk_ = (R)(-ctx->kappa), mk2 = (R)(-ctx->kappa * ctx->kappa);
+    const V *re = nullptr, *ro = nullptr;
+    switch (op) {
+    case CLOVER_OP_HOP_EO:
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(io, nullptr, oe, one, 0, XM_NONE, 0), B, st, nullptr));
+        re = oe;
+        break;
+    case CLOVER_OP_HOP_OE:
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(ie, nullptr, oo, one, 1, XM_NONE, 0), B, st, nullptr));
+        ro = oo;
+        break;
+    case CLOVER_OP_HOP_FULL:
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(io, nullptr, oe, one, 0, XM_NONE, 0), B, st, nullptr));
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(ie, nullptr, oo, one, 1, XM_NONE, 0), B, st, nullptr));
+        re = oe; ro = oo;
+        break;
+    case CLOVER_OP_CLOVER:
+    case CLOVER_OP_CLOVER_INV:
+        CLV_CHECK(launch_clover<R>(ctx, ie, oe, 0, op == CLOVER_OP_CLOVER_INV, B, st));
+        CLV_CHECK(launch_clover<R>(ctx, io, oo, 1, op == CLOVER_OP_CLOVER_INV, B, st));
+        re = oe; ro = oo;
+        break;
+    case CLOVER_OP_D_FULL:
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(io, ie, oe, mk_, 0, XM_CLOVER, 0), B, st, nullptr));
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(ie, io, oo, mk_, 1, XM_CLOVER, 0), B, st, nullptr));
+        re = oe; ro = oo;
+        break;
+    case CLOVER_OP_MHAT:
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(ie, nullptr, tmp, one, 1, XM_NONE, 1), B, st, nullptr));
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(tmp, ie, oe, mk2, 0, XM_CLOVER, 0), B, st, nullptr));
+        re = oe;
+        break;
+    default:
+        set_error("dslash_apply: unknown op %d", op);
+        return CLOVER_EINVAL;
+    }
+    CLV_CHECK((reorder_out<R, R>(g, out, re, ro, B, st)));
+    return 0;
+}
+
+int apply_op(clover_ctx *ctx, int op, int precision, const void *in, void *out, int n_rhs, cudaStream_t st)
+{
+    CLV_CHECK(ensure_work(ctx, std::min(8, ctx->max_rhs), 4, false));
+    const size_t per_rhs = (size_t)2 * ctx->geom.Vh * 24;
+    int lastB = -1;
+    for (int done = 0; done < n_rhs;) {
+        const int B = next_batch(n_rhs - done, ctx->max_rhs);
+        if (B != lastB) CLV_CHECK(clear_fields(ctx->work, ctx->geom, B, st));
+        lastB = B;
+        if (precision == 32) CLV_CHECK(apply_chunk<float>(ctx, op, (const float *)in + done * per_rhs, (float *)out + done * per_rhs, B, st));
+        else CLV_CHECK(apply_chunk<double>(ctx, op, (const double *)in + done * per_rhs, (double *)out + done * per_rhs, B, st));
+        done += B;
+    }
+    return 0;
+}
+
+// ---- kernel benchmark on internal-layout scratch fields ----------------------------------------------------------
+template <typename R> __global__ void fill_kernel(R *f, size_t n, unsigned salt)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        unsigned h = (unsigned)i * 2654435761u + salt;
+        h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+        f[i] = (R)((int)(h & 0xffff) - 32768) * (R)(1.0 / 32768.0);
+    }
+}
+
+template <typename R> static int bench_impl(clover_ctx *ctx, int kernel, int B, int reps, int flush_l2, float *ms_out, cudaStream_t st)
+{
+    typedef typename Vec<R>::T V;
+    SolveWork *W = ctx->work;
+    const Geom &g = ctx->geom;
+    V *f[4];
+    for (int i = 0; i < 4; i++) f[i] = sizeof(R) == 8 ? (V *)W->f64[i] : (V *)W->sl[i];
+    CLV_CHECK(clear_fields(W, g, B, st));
+    const size_t nreal = (size_t)((unsigned)g.Vh * B / 32u) * 32u * 24u;  // whole lane blocks only: padding lanes stay zero
+    for (int i = 0; i < 3; i++) fill_kernel<R><<<1184, 256, 0, st>>>((R *)f[i], nreal, 17u * i + 1u);
+    CLV_CUDA(cudaGetLastError());
+    const size_t flush_bytes = (size_t)256 << 20;
+    if (flush_l2 && !W->flush) CLV_CUDA(cudaMalloc(&W->flush, flush_bytes));
+    DslashArgs<R> a;
+    const R k2 = (R)(-ctx->kappa * ctx->kappa);
+    switch (kernel) {
+    case CLOVER_KERNEL_HOP: a = dargs<R>(f[0], nullptr, f[3], (R)1, 0, XM_NONE, 0); break;
+    case CLOVER_KERNEL_AINV_HOP: a = dargs<R>(f[0], nullptr, f[3], (R)1, 1, XM_NONE, 1); break;
+    case CLOVER_KERNEL_A_MINUS_HOP: a = dargs<R>(f[0], f[1], f[3], k2, 0, XM_CLOVER, 0, DOT_X, nullptr, W->partial); break;
+    default: set_error("clover_bench_kernel: unknown kernel %d", kernel); return CLOVER_EINVAL;
+    }
+    double total = 0;
+    for (int it = -3; it < reps; it++) {  // 3 warm-up launches
+        if (flush_l2) CLV_CUDA(cudaMemsetAsync(W->flush, it & 0xff, flush_bytes, st));
+        CLV_CUDA(cudaEventRecord(W->ev[0], st));
+        CLV_CHECK(launch_dslash<R>(ctx, a, B, st, nullptr));
+        CLV_CUDA(cudaEventRecord(W->ev[1], st));
+        CLV_CUDA(cudaEventSynchronize(W->ev[1]));
+        float ms;
+        CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[0], W->ev[1]));
+        if (it >= 0) total += ms;
+    }
+    *ms_out = (float)(total / reps);
+    return 0;
+}
+
+int bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms, cudaStream_t st)
+{
+    CLV_CHECK(ensure_work(ctx, n_rhs, 4, false));
+    return precision == 32 ? bench_impl<float>(ctx, kernel, n_rhs, reps, flush_l2, ms, st) : bench_impl<double>(ctx, kernel, n_rhs, reps, flush_l2, ms, st);
+}
+
+}  // namespace clv

@@ -1,0 +1,191 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's, in the scale-normalised reading R9 of DESIGN.md:
+max|gpu - oracle| / max|oracle| <= 1e-13 (fp64) / 1e-6 (fp32); solutions <= 1e-8 relative at an oracle-computed
+true residual <= 1e-10; Z4 noise bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1405_4524_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1405_4524_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def nerr(got, want):
+    return np.abs(got - want).max() / np.abs(want).max()
+
+
+class Setup:
+    def __init__(self, B, dims, eps, kappa, csw, seed, bc=(1, 1, 1, -1), recon=18, max_rhs=8):
+        self.dims, self.kappa, self.csw, self.bc = dims, kappa, csw, bc
+        self.U = wl.gauge_links(dims, eps, seed)
+        self.A = oracle.clover_matrix(self.U, kappa, csw)
+        self.Ainv = oracle.clover_inverse(self.A)
+        self.par = wl.parity_mask(dims)[..., None, None]
+        self.ctx = B.Clover(dev(self.U), kappa, csw, bc=bc, recon=recon, max_rhs=max_rhs)
+
+    def ref(self, B, op, psi):
+        e, o = (self.par == 0), (self.par == 1)
+        H = lambda v: oracle.hop(self.U, self.bc, v)
+        if op == B.OP_HOP_EO:
+            return e * H(o * psi)
+        if op == B.OP_HOP_OE:
+            return o * H(e * psi)
+        if op == B.OP_HOP_FULL:
+            return H(psi)
+        if op == B.OP_CLOVER:
+            return oracle.site_matvec(self.A, psi)
+        if op == B.OP_CLOVER_INV:
+            return oracle.site_matvec(self.Ainv, psi)
+        if op == B.OP_D_FULL:
+            return oracle.apply_D(self.U, self.A, self.bc, self.kappa, psi)
+        if op == B.OP_MHAT:
+            xe = e * psi
+            t = oracle.site_matvec(self.Ainv, o * H(xe))
+            return e * (oracle.site_matvec(self.A, xe) - self.kappa ** 2 * H(t))
+        raise ValueError(op)
+
+
+ALL_OPS = range(7)
+
+
+@pytest.mark.parametrize("dims,bc,n_rhs", [
+    ((4, 4, 4, 8), (1, 1, 1, -1), 1),
+    ((4, 6, 8, 10), (1, 1, 1, -1), 3),      # anisotropic: catches index-order bugs; 3 rhs = batches 2 + 1
+    ((2, 2, 2, 2), (1, 1, 1, -1), 8),       # x+mu == x-mu, padded lane blocks
+    ((6, 4, 2, 4), (-1, 1, -1, 1), 5),      # antiperiodic in x and z, Xh odd
+    ((8, 8, 8, 16), (1, 1, 1, 1), 8),       # the paper's periodic-in-time choice
+])
+def test_dslash_ops_fp64_and_fp32(B, dims, bc, n_rhs):
+    S = Setup(B, dims, 0.4, 0.118, 1.5, seed=101, bc=bc)
+    psi = wl.random_spinor(dims, 102, n_rhs)
+    for op in ALL_OPS:
+        want = np.stack([S.ref(B, op, psi[r]) for r in range(n_rhs)])
+        got = S.ctx.dslash_apply(op, dev(psi)).cpu().numpy()
+        assert nerr(got, want) < 1e-13, (op, "fp64", nerr(got, want))
+        got32 = S.ctx.dslash_apply(op, dev(psi.astype(np.complex64))).cpu().numpy()
+        assert got32.dtype == np.complex64
+        assert nerr(got32, want) < 1e-6, (op, "fp32", nerr(got32, want))
+    S.ctx.close()
+
+
+def test_dslash_recon12_fp32(B):
+    dims = (4, 6, 8, 10)
+    S = Setup(B, dims, 0.5, 0.115, 1.8, seed=111, recon=12)
+    psi = wl.random_spinor(dims, 112, 4)
+    for op in ALL_OPS:
+        want = np.stack([S.ref(B, op, psi[r]) for r in range(4)])
+        got32 = S.ctx.dslash_apply(op, dev(psi.astype(np.complex64))).cpu().numpy()
+        assert nerr(got32, want) < 1e-6, (op, nerr(got32, want))
+        got = S.ctx.dslash_apply(op, dev(psi)).cpu().numpy()       # fp64 links stay uncompressed
+        assert nerr(got, want) < 1e-13
+    S.ctx.close()
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 8), (8, 8, 8, 16), (6, 4, 2, 4)])
+def test_noise_bit_exact(B, dims):
+    s = wl.INV_SQRT2
+    for dil in (0, 1):
+        for off in (0, 5):
+            want = oracle.noise_fill(dims, 2001, 3, rhs_offset=off, time_dilution=dil, scale=s)
+            got = B.noise_fill(dims, 2001, 3, rhs_offset=off, time_dilution=dil, scale=s).cpu().numpy()
+            assert np.array_equal(got.view(np.uint64), want.view(np.uint64))
+            want32 = oracle.noise_fill(dims, 2001, 3, rhs_offset=off, time_dilution=dil, scale=s, dtype=np.float32)
+            got32 = B.noise_fill(dims, 2001, 3, rhs_offset=off, time_dilution=dil, scale=s, dtype=torch.complex64).cpu().numpy()
+            assert np.array_equal(got32.view(np.uint32), want32.view(np.uint32))
+
+
+def _check_solutions(S, eta, psi, infos, tol=1e-10, oracle_tol=1e-12, which=None):
+    n = eta.shape[0]
+    for r in range(n):
+        # oracle-computed true residual of the GPU solution
+        res = np.linalg.norm(eta[r] - oracle.apply_D(S.U, S.A, S.bc, S.kappa, psi[r])) / np.linalg.norm(eta[r])
+        assert res <= tol, (r, res)
+        assert infos[r]["status"] == 0 and abs(infos[r]["true_resid"] - res) <= 1e-3 * res + 1e-14
+    for r in (which if which is not None else range(n)):
+        want, info = oracle.bicgstab(S.U, S.A, S.bc, S.kappa, eta[r], tol=oracle_tol)
+        assert info["status"] == 0
+        assert np.linalg.norm(psi[r] - want) / np.linalg.norm(want) < 1e-8
+        assert nerr(psi[r], want) < 1e-8
+
+
+def test_solve_cfg0_fp64(B):
+    c = wl.CONFIGS[0]
+    S = Setup(B, c["dims"], c["eps"], c["kappa"], c["csw"], c["gauge_seed"])
+    eta = oracle.noise_fill(c["dims"], c["noise_seed"], 1, scale=wl.INV_SQRT2)
+    psi, infos, bad = S.ctx.solve(dev(eta), tol=wl.TOL, batch=1, mixed=False)
+    assert bad == 0
+    _check_solutions(S, eta, psi.cpu().numpy(), infos)
+    S.ctx.close()
+
+
+@pytest.mark.parametrize("mixed,batch", [(False, 4), (True, 4), (True, 2), (True, 1)])
+def test_solve_cfg1_batched(B, mixed, batch):
+    c = wl.CONFIGS[1]
+    S = Setup(B, c["dims"], c["eps"], c["kappa"], c["csw"], c["gauge_seed"])
+    eta = B.noise_fill(c["dims"], c["noise_seed"], 4, scale=wl.INV_SQRT2)
+    psi, infos, bad = S.ctx.solve(eta, tol=wl.TOL, batch=batch, mixed=mixed)
+    assert bad == 0
+    _check_solutions(S, eta.cpu().numpy(), psi.cpu().numpy(), infos, which=[0, 3])
+    if mixed:
+        assert all(i["reliable_updates"] >= 1 for i in infos)
+    S.ctx.close()
+
+
+def test_solve_ragged_batches_and_dilution_recon12(B):
+    """cfg2/cfg4-like parameters on a small lattice: 7 sources in batches 4+2+1, time dilution, two-row links."""
+    dims = (8, 8, 8, 16)
+    S = Setup(B, dims, 0.5, 0.115, 1.8, seed=1004, recon=12)
+    eta = B.noise_fill(dims, 2004, 7, rhs_offset=9, time_dilution=1, scale=wl.INV_SQRT2)
+    psi, infos, bad = S.ctx.solve(eta, tol=wl.TOL, batch=4, mixed=True)
+    assert bad == 0
+    _check_solutions(S, eta.cpu().numpy(), psi.cpu().numpy(), infos, which=[0, 6])
+    # host-buffer entry gives the same answer
+    psi_h, infos_h, bad_h = S.ctx.solve_host(eta.cpu().pin_memory(), tol=wl.TOL, batch=4, mixed=True)
+    assert bad_h == 0 and torch.equal(psi_h, psi.cpu())
+    S.ctx.close()
+
+
+def test_solve_point_source_free_field(B):
+    """Unit links, delta source: the sparse r0 that breaks a plain BiCGStab down (the oracle restarts there)."""
+    dims = (4, 4, 4, 8)
+    U = wl.unit_links(dims)
+    ctx = B.Clover(dev(U), 0.12, 1.0)
+    eta = np.zeros((2, 8, 4, 4, 4, 4, 3), dtype=complex)
+    eta[0, 0, 0, 0, 0, 2, 1] = 1
+    eta[1, 3, 1, 2, 3, 0, 0] = 1
+    psi, infos, bad = ctx.solve(dev(eta), tol=1e-10, batch=2, mixed=True)
+    A = oracle.clover_matrix(U, 0.12, 1.0)
+    for r in range(2):
+        res = np.linalg.norm(eta[r] - oracle.apply_D(U, A, (1, 1, 1, -1), 0.12, psi[r].cpu().numpy())) / np.linalg.norm(eta[r])
+        assert infos[r]["status"] in (0, 2)
+        if infos[r]["status"] == 0:
+            assert res <= 1e-10
+    ctx.close()
+
+
+def test_zero_source_and_errors(B):
+    dims = (4, 4, 4, 8)
+    S = Setup(B, dims, 0.2, 0.12, 1.0, seed=1)
+    eta = torch.zeros((2, 8, 4, 4, 4, 4, 3), dtype=torch.complex128, device="cuda")
+    eta[1] = B.noise_fill(dims, 3, 1)[0]
+    psi, infos, bad = S.ctx.solve(eta, batch=2)
+    assert bad == 0 and torch.count_nonzero(psi[0]) == 0 and infos[0]["true_resid"] == 0.0
+    with pytest.raises(B.CloverError):
+        S.ctx.solve(eta, batch=3)
+    with pytest.raises(B.CloverError):
+        B.Clover(dev(wl.unit_links((4, 4, 4, 8)))[:, :, :, :, :3].contiguous(), 0.12, 1.0)   # odd X
+    with pytest.raises(B.CloverError):
+        B.Clover(dev(S.U), 0.12, 1.0, recon=8)
+    S.ctx.close()
