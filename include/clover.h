@@ -115,10 +115,14 @@ int clover_bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, i
                         void *stream);
 
 /* Counters of the last clover_solve* call on this context: kernels launched, and device time (ms) spent
- * in the phases {reorder in/out, source prep, iteration, reliable updates, reconstruct+verify}. */
+ * in the phases {reorder in/out, source prep, iteration, reliable updates, reconstruct+verify}, summed over batches. */
 typedef struct {
     long long kernel_launches;
     double ms_total, ms_reorder, ms_prep, ms_iterate, ms_reliable, ms_finish;
+    /* the two Dslash kernels of the sloppy (iteration-precision) Mhat, timed launch by launch with CUDA events on `stream`:
+       ainv_hop = t_o = A_oo^-1 H_oe x_e ;  a_minus_hop = y_e = A_ee x_e - kappa^2 H_eo t_o with its dot-product epilogue */
+    long long n_ainv_hop, n_a_minus_hop;
+    double ms_ainv_hop, ms_a_minus_hop;
 } clover_solve_stats;
 int clover_get_stats(const clover_ctx *ctx, clover_solve_stats *out);
 

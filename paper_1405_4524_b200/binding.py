@@ -33,7 +33,8 @@ class RhsInfo(ctypes.Structure):
 class SolveStats(ctypes.Structure):
     _fields_ = [("kernel_launches", ctypes.c_longlong), ("ms_total", ctypes.c_double), ("ms_reorder", ctypes.c_double),
                 ("ms_prep", ctypes.c_double), ("ms_iterate", ctypes.c_double), ("ms_reliable", ctypes.c_double),
-                ("ms_finish", ctypes.c_double)]
+                ("ms_finish", ctypes.c_double), ("n_ainv_hop", ctypes.c_longlong), ("n_a_minus_hop", ctypes.c_longlong),
+                ("ms_ainv_hop", ctypes.c_double), ("ms_a_minus_hop", ctypes.c_double)]
 
 
 _vp, _ip, _i, _d = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.c_int, ctypes.c_double
@@ -103,9 +104,9 @@ class Clover:
         _check(_lib.clover_create(ctypes.byref(self._ctx), gauge.data_ptr(), _i4(self.dims), kappa, csw, _i4(bc), ctypes.byref(opts), _stream()))
 
     def close(self):
-        if getattr(self, "_ctx", None):
+        if getattr(self, "_ctx", None) and _lib is not None:   # _lib is None during interpreter shutdown
             _lib.clover_destroy(self._ctx)
-            self._ctx = None
+        self._ctx = None
 
     __del__ = close
 

@@ -24,6 +24,7 @@ struct SolveWork {
     size_t stage_bytes = 0;
     void *flush = nullptr;
     cudaEvent_t ev[6] = {};
+    cudaEvent_t kev[6] = {};   // per-launch timing of the two sloppy Mhat calls of an iteration: 2 x (start, mid, end)
     bool have_ev = false;
 };
 
@@ -41,7 +42,7 @@ void free_work(clover_ctx *ctx)
     cudaFree(W->stage_in);
     cudaFree(W->stage_out);
     cudaFree(W->flush);
-    if (W->have_ev) for (int i = 0; i < 6; i++) cudaEventDestroy(W->ev[i]);
+    if (W->have_ev) for (int i = 0; i < 6; i++) { cudaEventDestroy(W->ev[i]); cudaEventDestroy(W->kev[i]); }
     delete W;
     ctx->work = nullptr;
 }
@@ -93,7 +94,7 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
         }
     }
     if (!W->have_ev) {
-        for (int i = 0; i < 6; i++) CLV_CUDA(cudaEventCreate(&W->ev[i]));
+        for (int i = 0; i < 6; i++) { CLV_CUDA(cudaEventCreate(&W->ev[i])); CLV_CUDA(cudaEventCreate(&W->kev[i])); }
         W->have_ev = true;
     }
     CLV_CUDA(cudaDeviceSynchronize());  // the memsets above ran on the legacy stream
@@ -126,11 +127,14 @@ template <typename R> static DslashArgs<R> dargs(const typename Vec<R>::T *in, c
 // out_e = Mhat in_e, optional fused dot products; tmp is an odd-parity scratch field
 template <typename R>
 static int mhat(clover_ctx *ctx, int B, const typename Vec<R>::T *in, typename Vec<R>::T *tmp, typename Vec<R>::T *out, int dot, const typename Vec<R>::T *w,
-                double *partial, int *grid, cudaStream_t st)
+                double *partial, int *grid, cudaStream_t st, cudaEvent_t *kev = nullptr)
 {
     const R k2 = (R)(-ctx->kappa * ctx->kappa);
+    if (kev) CLV_CUDA(cudaEventRecord(kev[0], st));
     CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(in, nullptr, tmp, (R)1, 1, XM_NONE, 1), B, st, nullptr));
+    if (kev) CLV_CUDA(cudaEventRecord(kev[1], st));
     CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(tmp, in, out, k2, 0, XM_CLOVER, 0, dot, w, partial), B, st, grid));
+    if (kev) CLV_CUDA(cudaEventRecord(kev[2], st));
     ctx->stats.kernel_launches += 2;
     return 0;
 }
@@ -190,15 +194,21 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     auto any_update = [&]() { for (int i = 0; i < B; i++) if (!W->sc_host[i].done && W->sc_host[i].want_update) return true; return false; };
     double ms_reliable = 0;
     while (!all_done() && iters < max_iter) {
-        CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_W, r0, W->partial, &grid, st));
+        CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_W, r0, W->partial, &grid, st, W->kev));
         CLV_CHECK(blas_scalar_step(bc, SC_ALPHA, grid, tol2, delta2));
         CLV_CHECK(blas_s_update<R>(bc, r, v, s));
-        CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_X, nullptr, W->partial, &grid, st));
+        CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_X, nullptr, W->partial, &grid, st, W->kev + 3));
         CLV_CHECK(blas_scalar_step(bc, SC_OMEGA, grid, tol2, delta2));
         CLV_CHECK(blas_xr_update<R>(bc, x, r, p, s, t, r0, &nb));
         CLV_CHECK(blas_scalar_step(bc, SC_RHO, nb, tol2, delta2));
         CLV_CHECK(fetch_scalars(W, B, st));
         iters++;
+        for (int h = 0; h < 2; h++) {
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h], W->kev[3 * h + 1])); ctx->stats.ms_ainv_hop += ms;
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h + 1], W->kev[3 * h + 2])); ctx->stats.ms_a_minus_hop += ms;
+        }
+        ctx->stats.n_ainv_hop += 2;
+        ctx->stats.n_a_minus_hop += 2;
         if (any_update() || iters == max_iter) {
             // reliable update: y += x, x = 0, r = b - Mhat y in fp64 (S 8(c) O6')
             CLV_CUDA(cudaEventRecord(W->ev[4], st));
