@@ -125,6 +125,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel-bench", action="store_true", help="only time the three Dslash kernels alone (fp32/fp64, B = 1 and batch) and print them")
     ap.add_argument("--reps", type=int, default=20)
+    ap.add_argument("--kb-filter", default="", help="comma-separated substrings; with --kernel-bench only time kernels whose name contains one")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -168,6 +169,8 @@ def main():
             g = cfg["recon"] if prec == 32 else 18
             for nr in sorted({1, batch}):
                 for k, name, fl in ((B.KERNEL_HOP, "hop", 1320), (B.KERNEL_AINV_HOP, "ainv_hop", 1824), (B.KERNEL_A_MINUS_HOP, "a_minus_hop", 1872)):
+                    if args.kb_filter and not any(f in f"fp{prec}_{name}_b{nr}" for f in args.kb_filter.split(",")):
+                        continue
                     t = ctx.bench_kernel(k, prec, nr, reps=args.reps, flush_l2=True) * 1e-3
                     bm = (8 * g * b + (72 * b if k else 0)) / nr + 24 * b * (3 if k == B.KERNEL_A_MINUS_HOP else 2)
                     res[f"fp{prec}_{name}_b{nr}"] = {"us": round(t * 1e6, 2), "bytes_per_site_rhs": bm, "gbs": round(bm * Vh * nr / t / 1e9, 1),

@@ -13,7 +13,13 @@
 
 namespace clv {
 
-constexpr int DSLASH_BLOCK = 128;
+#ifndef CLV_DSLASH_BLOCK
+#define CLV_DSLASH_BLOCK 128
+#endif
+#ifndef CLV_DSLASH_MINB
+#define CLV_DSLASH_MINB 4 // <= 128 registers: measured best (ptxas keeps more loads in flight than with no hint; profiles/r1_tuning.md)
+#endif
+constexpr int DSLASH_BLOCK = CLV_DSLASH_BLOCK;
 
 template <typename R, int MU, int FWD> __device__ __forceinline__ void project(const cx<R> psi[12], cx<R> h[6])
 {
@@ -150,7 +156,7 @@ template <int B, int BLOCK> __device__ __forceinline__ void block_reduce_rhs(dou
 }
 
 template <typename R, int B, int RECON, int XMODE, int PINV, int DOT>
-__global__ void __launch_bounds__(DSLASH_BLOCK) dslash_kernel(const Geom g, const OpData<R> op, const DslashArgs<R> a)
+__global__ void __launch_bounds__(DSLASH_BLOCK, CLV_DSLASH_MINB) dslash_kernel(const Geom g, const OpData<R> op, const DslashArgs<R> a)
 {
     const unsigned j = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
     const bool active = j < (unsigned)g.Vh * B;

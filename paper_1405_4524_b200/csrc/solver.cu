@@ -150,7 +150,7 @@ static double reliable_delta()
 {
     const char *e = getenv("CLOVER_DELTA");  // tuning/debug knob only
     const double d = e ? atof(e) : 0.0;
-    return (d > 0.0 && d < 1.0) ? d : 0.05;
+    return (d > 0.0 && d < 1.0) ? d : 0.01;
 }
 
 template <typename R>
