@@ -150,12 +150,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    from paper_1405_4524_b200 import sharding
+
     def max_over_ranks(x):
-        if not dist:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return sharding.max_over_ranks(x, device="cuda")
 
     dims, n_rhs, batch = cfg["dims"], cfg["n_rhs"], cfg["batch"]
     X, Y, Z, T = dims
@@ -179,7 +177,7 @@ def main():
         ctx.close()
         return
     # weak scaling: every rank solves its own n_rhs sources (distinct noise streams), replicas of the operator, no collective
-    offset = rank * n_rhs
+    offset = sharding.source_offset(rank, n_rhs)
     eta = torch.empty((n_rhs, T, Z, Y, X, 4, 3), dtype=torch.complex128, device="cuda")
     psi = torch.empty_like(eta)
     launches = 0
@@ -215,8 +213,7 @@ def main():
     barrier()
     sampler.stop_flag = True
     ms = max_over_ranks(e0.elapsed_time(e1))
-    sec_per_source = ms * 1e-3 / (args.steps * n_rhs)       # every rank solves n_rhs per step concurrently
-    value = sec_per_source / world                          # whole-job: world * n_rhs sources per step
+    value = sharding.whole_job_seconds_per_source(ms, args.steps, n_rhs, world)   # world * n_rhs sources per step
 
     # ---- roofline of the dominant kernel: the fused fp32 Dslash y_e = A x_e - kappa^2 H_eo t_o (+dots) of the iteration ----
     peaks, peak_kind = measured_peaks()
