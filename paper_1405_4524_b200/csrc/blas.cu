@@ -201,13 +201,17 @@ __device__ __forceinline__ double2 st_z(zs z) { return make_double2(z.re, z.im);
 __device__ __forceinline__ bool finite_z(zs z) { return isfinite(z.re) && isfinite(z.im); }
 
 // one block per rhs: sum partial[(b*B + rhs)*4 + c] over b < nblocks in a fixed order, then thread 0 updates the scalars.
+constexpr int SC_SLICES = 32;
 __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblocks, const double *__restrict__ partial, RhsScalars *sc, double tol2,
-                                                     double delta2)
+                                                     double delta2, double *stage, unsigned *ticket)
 {
     __shared__ double sm[256][3];
-    const int rhs = blockIdx.x;
+    __shared__ bool last;
+    const int rhs = blockIdx.x, slice = blockIdx.y;
+    // stage 1: this block sums its contiguous slice of the per-block partials (fixed order)
+    const int per = (nblocks + SC_SLICES - 1) / SC_SLICES, lo = slice * per, hi = min(nblocks, lo + per);
     double a0 = 0, a1 = 0, a2 = 0;
-    for (int b = threadIdx.x; b < nblocks; b += 256) {
+    for (int b = lo + threadIdx.x; b < hi; b += 256) {
         const double *q = partial + ((size_t)b * B + rhs) * 4;
         a0 += q[0];
         a1 += q[1];
@@ -225,8 +229,26 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         }
         __syncthreads();
     }
-    if (threadIdx.x != 0) return;
-    const double d0 = sm[0][0], d1 = sm[0][1], d2 = sm[0][2];
+    if (threadIdx.x == 0) {
+        double *o = stage + ((size_t)rhs * SC_SLICES + slice) * 4;
+        o[0] = sm[0][0];
+        o[1] = sm[0][1];
+        o[2] = sm[0][2];
+        __threadfence();
+        last = (atomicAdd(ticket + rhs, 1u) == SC_SLICES - 1);
+    }
+    __syncthreads();
+    if (!last || threadIdx.x != 0) return;
+    // stage 2 (last block of this rhs to arrive): sum the slices in order, then the scalar recurrences
+    __threadfence();
+    ticket[rhs] = 0;
+    double d0 = 0, d1 = 0, d2 = 0;
+    for (int k = 0; k < SC_SLICES; k++) {
+        const volatile double *o = stage + ((size_t)rhs * SC_SLICES + k) * 4;
+        d0 += o[0];
+        d1 += o[1];
+        d2 += o[2];
+    }
     RhsScalars &q = sc[rhs];
     const zs zero{0., 0.};
     switch (step) {
@@ -241,6 +263,7 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         q.r2 = q.maxr2 = q.true_r2 = d0;
         q.alpha = q.omega = q.beta = make_double2(0., 0.);
         q.want_update = 0;
+        q.claim = 0;
         if (!(q.eta2 > 0.) || d0 <= tol2 * q.eta2) q.done = 1;  // zero source or already converged
         if (!isfinite(d0)) { q.done = 1; q.status = 3; }
         break;
@@ -267,13 +290,15 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
     case SC_RHO: {  // (d0,d1) = <r0, r>, d2 = ||r||^2
         zs be = zero;
         q.want_update = 0;
+        q.claim = 0;
         if (!q.done) {
             const zs rho1{d0, d1}, om = ld_z(q.omega), rho = ld_z(q.rho);
             q.r2 = d2;
             if (d2 > q.maxr2) q.maxr2 = d2;
             if (!isfinite(d2) || !finite_z(rho1)) { q.done = 1; q.status = 3; }
             else {
-                if (d2 < delta2 * q.maxr2 || d2 <= tol2 * q.eta2) q.want_update = 1;
+                if (d2 < delta2 * q.maxr2) q.want_update = 1;
+                q.claim = (d2 <= tol2 * q.eta2) ? 1 : 0;
                 const double om2 = om.re * om.re + om.im * om.im, rh2 = rho.re * rho.re + rho.im * rho.im;
                 if (!(om2 > 0.) || !(rh2 > 0.)) q.want_update = 1;  // stagnation: let the fp64 residual decide, beta = 0 restarts p = r
                 else be = zmul(zdiv(rho1, rho), zdiv(ld_z(q.alpha), om));
@@ -286,6 +311,7 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
     }
     case SC_TRUE:  // d0 = ||b - Mhat y||^2 in fp64
         q.true_r2 = d0;
+        q.claim = 0;
         if (!q.done) {
             q.r2 = q.maxr2 = d0;
             q.want_update = 0;
@@ -360,7 +386,7 @@ int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, cons
 }
 int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2)
 {
-    scalar_kernel<<<c.B, 256, 0, c.st>>>(step, c.B, nblocks, c.partial, c.sc, tol2, delta2);
+    scalar_kernel<<<dim3(c.B, SC_SLICES), 256, 0, c.st>>>(step, c.B, nblocks, c.partial, c.sc, tol2, delta2, c.stage, c.ticket);
     BLAS_LAUNCHED(c);
     CLV_CUDA(cudaGetLastError());
     return 0;

@@ -13,6 +13,8 @@ struct BlasCtx {
     RhsScalars *sc;    // device, B entries
     double *partial;   // device, [blocks][B][4]
     int max_partial_blocks;
+    double *stage;     // device, [8 rhs][32 slices][4]: second-level partials of the scalar kernels
+    unsigned *ticket;  // device, [8]: arrival counters of the scalar kernels (zero between launches)
     cudaStream_t st;
     long long *launches;
 };

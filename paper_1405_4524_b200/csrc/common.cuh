@@ -67,6 +67,17 @@ struct Geom {
 
 // vector index of (j, k) in a lane-blocked field with NK vectors per entry
 __host__ __device__ __forceinline__ unsigned lb_index(unsigned j, int k, int NK) { return ((j >> 5) * NK + k) * 32u + (j & 31u); }
+// index (in complex elements) of complex element k of entry cb in a lane-blocked complex field with NK elements per entry.
+// fp64: one double2 per (k, lane).  fp32: elements are packed in pairs so that a thread fetches two of them with one
+// 16-byte load: per 32-entry block, NK/2 float4 rows [k/2][lane] followed, if NK is odd, by one float2 row [lane].
+template <typename R> __host__ __device__ __forceinline__ unsigned cplx_index(unsigned cb, int k, int NK)
+{
+    if (sizeof(R) == 8) return lb_index(cb, k, NK);
+    const unsigned base = (cb >> 5) * 32u * NK, lane = cb & 31u;
+    const int n4 = NK / 2;
+    return (k < 2 * n4) ? base + ((unsigned)(k >> 1) * 32u + lane) * 2u + (k & 1) : base + (unsigned)n4 * 64u + lane;
+}
+
 // number of 32-lane blocks needed for n entries
 __host__ __device__ __forceinline__ unsigned lb_blocks(unsigned n) { return (n + 31u) >> 5; }
 
@@ -149,26 +160,41 @@ __device__ __forceinline__ void store_spinor(double2 *__restrict__ f, unsigned j
     for (int k = 0; k < 12; k++) p[32 * k] = make_double2(psi[k].re, psi[k].im);
 }
 
-// complex element k of entry cb in a lane-blocked complex field with NK elements per entry
-template <typename C> __device__ __forceinline__ C load_c(const C *__restrict__ f, unsigned cb, int k, int NK)
+// link at cb: RECON = 18 -> 9 stored complex; RECON = 12 -> rows 0,1 stored, row 2 = conj(row0 x row1) rebuilt by third_row()
+// at the point of use (not at the load, so that loads can be issued a direction ahead)
+template <typename R, int RECON> __device__ __forceinline__ void third_row(cx<R> u[9])
 {
-    return __ldg(f + lb_index(cb, k, NK));
-}
-
-// link at cb: RECON = 18 -> 9 stored complex; RECON = 12 -> rows 0,1 stored, row 2 = conj(row0 x row1)
-template <typename R, int RECON> __device__ __forceinline__ void load_link(const typename Vec<R>::C *__restrict__ f, unsigned cb, cx<R> u[9])
-{
-    constexpr int NK = RECON / 2;
-    const typename Vec<R>::C *p = f + lb_index(cb, 0, NK);
-#pragma unroll
-    for (int k = 0; k < NK; k++) {
-        typename Vec<R>::C v = __ldg(p + 32 * k);
-        u[k] = mk<R>(v.x, v.y);
-    }
     if (RECON == 12) {
         u[6] = conj(u[1] * u[5] - u[2] * u[4]);
         u[7] = conj(u[2] * u[3] - u[0] * u[5]);
         u[8] = conj(u[0] * u[4] - u[1] * u[3]);
+    }
+}
+template <int RECON> __device__ __forceinline__ void load_link(const double2 *__restrict__ f, unsigned cb, cx<double> u[9])
+{
+    constexpr int NK = RECON / 2;
+    const double2 *p = f + lb_index(cb, 0, NK);
+#pragma unroll
+    for (int k = 0; k < NK; k++) {
+        double2 v = __ldg(p + 32 * k);
+        u[k] = mk<double>(v.x, v.y);
+    }
+}
+template <int RECON> __device__ __forceinline__ void load_link(const float2 *__restrict__ f, unsigned cb, cx<float> u[9])
+{
+    constexpr int NK = RECON / 2, N4 = NK / 2;
+    const float2 *blk = f + (cb >> 5) * 32u * NK;
+    const unsigned lane = cb & 31u;
+    const float4 *p4 = reinterpret_cast<const float4 *>(blk) + lane;
+#pragma unroll
+    for (int k = 0; k < N4; k++) {
+        float4 v = __ldg(p4 + 32 * k);
+        u[2 * k] = mk<float>(v.x, v.y);
+        u[2 * k + 1] = mk<float>(v.z, v.w);
+    }
+    if (NK & 1) {
+        float2 v = __ldg(blk + N4 * 64 + lane);
+        u[NK - 1] = mk<float>(v.x, v.y);
     }
 }
 

@@ -23,9 +23,9 @@ struct RhsScalars {
     double eta2;      // ||eta||^2 on the full lattice (stopping scale, R10)
     double true_r2;   // ||r||^2 at the last fp64 recomputation
     int done;         // 1 once the fp64 residual met the tolerance (rhs frozen)
-    int want_update;  // 1 if this rhs asks for a reliable update
+    int want_update;  // 1 if this rhs asks for a reliable update (||r|| < delta max||r||, or stagnation)
     int status;       // clover_rhs_info.status
-    int pad;
+    int claim;        // 1 if the iterated residual of this rhs meets the tolerance (to be confirmed in fp64)
 };
 
 struct SolveWork;  // solver.cu

@@ -66,54 +66,181 @@ template <typename R, int MU, int FWD> __device__ __forceinline__ void reconstru
     }
 }
 
+// ---- accumulation of one direction: acc += (g, -+ B^+ g), g = U h or U^+ h --------------------------------------
+// Generic (fp64) version: scalar complex arithmetic.
+template <typename R> struct HopAcc {
+    cx<R> acc[12];
+    __device__ __forceinline__ void zero()
+    {
+#pragma unroll
+        for (int i = 0; i < 12; i++) acc[i] = mk<R>(0, 0);
+    }
+    template <int MU, int FWD> __device__ __forceinline__ void add(const cx<R> h[6], const cx<R> u[9])
+    {
+        cx<R> gh[6];
+#pragma unroll
+        for (int s = 0; s < 2; s++)
+#pragma unroll
+            for (int a = 0; a < 3; a++) {
+                cx<R> t = mk<R>(0, 0);
+#pragma unroll
+                for (int b = 0; b < 3; b++) {
+                    if (FWD) fma_cx(t, u[a * 3 + b], h[s * 3 + b]);
+                    else fma_conj(t, u[b * 3 + a], h[s * 3 + b]);
+                }
+                gh[s * 3 + a] = t;
+            }
+        reconstruct<R, MU, FWD>(gh, acc);
+    }
+    __device__ __forceinline__ void finish(cx<R> out[12]) const
+    {
+#pragma unroll
+        for (int i = 0; i < 12; i++) out[i] = acc[i];
+    }
+};
+
+// fp32 version on Blackwell's packed f32x2 pipe (FFMA2 / FADD2, one issue slot for two FMAs).  The two spin
+// components of the half spinor are carried as a pair: the link acts on colour only, so each link element is a scalar
+// broadcast operand of FFMA2 (SASS `R.F32`), and the SU(3) x half-spinor product costs 36 FFMA2 instead of 72 FFMA.
+// Lower-spin accumulators are kept twice, in (2,3) order for mu = z,t and in (3,2) order for mu = x,y, so that
+// B^+ g never needs a lane swap; they are merged in finish().
+template <> struct HopAcc<float> {
+    float2 ure[3], uim[3];  // (acc[a], acc[3+a])         real / imaginary parts
+    float2 lre[3], lim[3];  // (acc[6+a], acc[9+a])       fed by mu = 2, 3
+    float2 xre[3], xim[3];  // (acc[9+a], acc[6+a])       fed by mu = 0, 1
+    __device__ __forceinline__ void zero()
+    {
+#pragma unroll
+        for (int a = 0; a < 3; a++) ure[a] = uim[a] = lre[a] = lim[a] = xre[a] = xim[a] = make_float2(0.f, 0.f);
+    }
+    template <int MU, int FWD> __device__ __forceinline__ void add(const cx<float> h[6], const cx<float> u[9])
+    {
+        float2 hre[3], him[3];
+#pragma unroll
+        for (int b = 0; b < 3; b++) {
+            hre[b] = make_float2(h[b].re, h[3 + b].re);
+            him[b] = make_float2(h[b].im, h[3 + b].im);
+        }
+        constexpr float s = FWD ? -1.f : 1.f;
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            float2 gre, gim;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                const cx<float> e = FWD ? u[a * 3 + b] : u[b * 3 + a];
+                const float ei = FWD ? e.im : -e.im;  // U^+ : conjugate
+                const float2 er2 = make_float2(e.re, e.re), ei2 = make_float2(ei, ei), nei2 = make_float2(-ei, -ei);
+                if (b == 0) {
+                    gre = __fmul2_rn(er2, hre[0]);
+                    gim = __fmul2_rn(er2, him[0]);
+                } else {
+                    gre = __ffma2_rn(er2, hre[b], gre);
+                    gim = __ffma2_rn(er2, him[b], gim);
+                }
+                gre = __ffma2_rn(nei2, him[b], gre);
+                gim = __ffma2_rn(ei2, hre[b], gim);
+            }
+            ure[a] = __fadd2_rn(ure[a], gre);
+            uim[a] = __fadd2_rn(uim[a], gim);
+            if (MU == 0) {  // acc2 += s i g1, acc3 += s i g0
+                xre[a] = __ffma2_rn(gim, make_float2(-s, -s), xre[a]);
+                xim[a] = __ffma2_rn(gre, make_float2(s, s), xim[a]);
+            } else if (MU == 1) {  // acc2 += s g1, acc3 -= s g0
+                xre[a] = __ffma2_rn(gre, make_float2(-s, s), xre[a]);
+                xim[a] = __ffma2_rn(gim, make_float2(-s, s), xim[a]);
+            } else if (MU == 2) {  // acc2 += s i g0, acc3 -= s i g1
+                lre[a] = __ffma2_rn(gim, make_float2(-s, s), lre[a]);
+                lim[a] = __ffma2_rn(gre, make_float2(s, -s), lim[a]);
+            } else {  // acc2 += s g0, acc3 += s g1
+                lre[a] = __ffma2_rn(gre, make_float2(s, s), lre[a]);
+                lim[a] = __ffma2_rn(gim, make_float2(s, s), lim[a]);
+            }
+        }
+    }
+    __device__ __forceinline__ void finish(cx<float> out[12]) const
+    {
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            out[a] = mk<float>(ure[a].x, uim[a].x);
+            out[3 + a] = mk<float>(ure[a].y, uim[a].y);
+            out[6 + a] = mk<float>(lre[a].x + xre[a].y, lim[a].x + xim[a].y);
+            out[9 + a] = mk<float>(lre[a].y + xre[a].x, lim[a].y + xim[a].x);
+        }
+    }
+};
+
+// One direction of the hop, split into its loads and its arithmetic so that the kernel can issue the loads of direction
+// d+1 before the arithmetic of direction d (explicit software pipelining; profiles/r1_tuning.md).
+template <typename R> struct HopIn {
+    cx<R> psi[12];
+    cx<R> u[9];
+    bool neg;
+};
 template <typename R, int B, int RECON, int MU, int FWD>
-__device__ __forceinline__ void hop_dir(const Geom &g, const OpData<R> &op, const typename Vec<R>::T *__restrict__ in, int p, int cb,
-                                        int rhs, const Coord &c, cx<R> acc[12])
+__device__ __forceinline__ void hop_load(const Geom &g, const OpData<R> &op, const typename Vec<R>::T *__restrict__ in, int p, int cb, int rhs,
+                                         const Coord &c, HopIn<R> &d)
 {
     bool wrap;
-    const int nb = neighbour<MU, FWD>(g, cb, c, wrap);
-    cx<R> psi[12], h[6], u[9], gh[6];
-    load_spinor(in, (unsigned)nb * B + rhs, psi);
+    int nb = neighbour<MU, FWD>(g, cb, c, wrap);
+#ifdef CLV_FAKE_NB
+    nb = cb;  // experiment only: all neighbours = own site (upper bound of L1 reuse)
+#endif
+    load_spinor(in, (unsigned)nb * B + rhs, d.psi);
     // (ternaries rather than op.gauge[p]: runtime indexing of a kernel parameter would force a local copy)
-    if (FWD) load_link<R, RECON>(p ? op.gauge[1][MU] : op.gauge[0][MU], cb, u);
-    else load_link<R, RECON>(p ? op.gauge[0][MU] : op.gauge[1][MU], nb, u);
-    project<R, MU, FWD>(psi, h);
-    if (wrap && g.bc[MU] < 0) {
+    if (FWD) load_link<RECON>(p ? op.gauge[1][MU] : op.gauge[0][MU], cb, d.u);
+    else load_link<RECON>(p ? op.gauge[0][MU] : op.gauge[1][MU], nb, d.u);
+    d.neg = wrap && g.bc[MU] < 0;
+}
+template <typename R, int RECON, int MU, int FWD> __device__ __forceinline__ void hop_compute(HopIn<R> &d, HopAcc<R> &acc)
+{
+    cx<R> h[6];
+    third_row<R, RECON>(d.u);
+    project<R, MU, FWD>(d.psi, h);
+    if (d.neg) {
 #pragma unroll
         for (int i = 0; i < 6; i++) h[i] = mk<R>(-h[i].re, -h[i].im);
     }
+    acc.template add<MU, FWD>(h, d.u);
+}
+
+// the 18 packed complex numbers of chirality block `blk` of one site (3 diagonal pairs, 15 lower off-diagonals)
+__device__ __forceinline__ void load_clover_block(const double2 *__restrict__ clov, unsigned cb, int blk, cx<double> m[18])
+{
+    const double2 *p = clov + lb_index(cb, 18 * blk, 36);
 #pragma unroll
-    for (int s = 0; s < 2; s++)
+    for (int k = 0; k < 18; k++) {
+        double2 v = __ldg(p + 32 * k);
+        m[k] = mk<double>(v.x, v.y);
+    }
+}
+__device__ __forceinline__ void load_clover_block(const float2 *__restrict__ clov, unsigned cb, int blk, cx<float> m[18])
+{
+    const float4 *p = reinterpret_cast<const float4 *>(clov + (cb >> 5) * 32u * 36u) + (cb & 31u) + 32 * 9 * blk;
 #pragma unroll
-        for (int a = 0; a < 3; a++) {
-            cx<R> t = mk<R>(0, 0);
-#pragma unroll
-            for (int b = 0; b < 3; b++) {
-                if (FWD) fma_cx(t, u[a * 3 + b], h[s * 3 + b]);
-                else fma_conj(t, u[b * 3 + a], h[s * 3 + b]);
-            }
-            gh[s * 3 + a] = t;
-        }
-    reconstruct<R, MU, FWD>(gh, acc);
+    for (int k = 0; k < 9; k++) {
+        float4 v = __ldg(p + 32 * k);
+        m[2 * k] = mk<float>(v.x, v.y);
+        m[2 * k + 1] = mk<float>(v.z, v.w);
+    }
 }
 
 // y (+)= M x for the two packed 6x6 Hermitian blocks of one site
 template <typename R, bool ACCUM>
 __device__ __forceinline__ void clover_mul(const typename Vec<R>::C *__restrict__ clov, unsigned cb, const cx<R> x[12], cx<R> y[12])
 {
-    const typename Vec<R>::C *p = clov + lb_index(cb, 0, 36);
 #pragma unroll
     for (int blk = 0; blk < 2; blk++) {
         const int o = 6 * blk;
+        cx<R> m[18];
+        load_clover_block(clov, cb, blk, m);
 #pragma unroll
         for (int k = 0; k < 3; k++) {
-            const typename Vec<R>::C d = __ldg(p + 32 * (18 * blk + k));
             if (ACCUM) {
-                y[o + 2 * k] = y[o + 2 * k] + d.x * x[o + 2 * k];
-                y[o + 2 * k + 1] = y[o + 2 * k + 1] + d.y * x[o + 2 * k + 1];
+                y[o + 2 * k] = y[o + 2 * k] + m[k].re * x[o + 2 * k];
+                y[o + 2 * k + 1] = y[o + 2 * k + 1] + m[k].im * x[o + 2 * k + 1];
             } else {
-                y[o + 2 * k] = d.x * x[o + 2 * k];
-                y[o + 2 * k + 1] = d.y * x[o + 2 * k + 1];
+                y[o + 2 * k] = m[k].re * x[o + 2 * k];
+                y[o + 2 * k + 1] = m[k].im * x[o + 2 * k + 1];
             }
         }
         int k = 3;
@@ -121,10 +248,8 @@ __device__ __forceinline__ void clover_mul(const typename Vec<R>::C *__restrict_
         for (int i = 1; i < 6; i++)
 #pragma unroll
             for (int j = 0; j < i; j++, k++) {
-                const typename Vec<R>::C v = __ldg(p + 32 * (18 * blk + k));
-                const cx<R> L = mk<R>(v.x, v.y);
-                fma_cx(y[o + i], L, x[o + j]);
-                fma_conj(y[o + j], L, x[o + i]);
+                fma_cx(y[o + i], m[k], x[o + j]);
+                fma_conj(y[o + j], m[k], x[o + i]);
             }
     }
 }
@@ -155,6 +280,41 @@ template <int B, int BLOCK> __device__ __forceinline__ void block_reduce_rhs(dou
     }
 }
 
+// L1 prefetch of everything the epilogue will read (clover blocks, xin, w): issued part-way through the hop so that the
+// epilogue's loads -- first touches of DRAM lines, at the end of a dependent chain -- do not stall the warp for a full
+// DRAM round trip with no registers left to overlap it.
+#ifndef CLV_PIPE
+#define CLV_PIPE 1
+#endif
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+template <typename R, int XMODE, int PINV, int DOT>
+__device__ __forceinline__ void prefetch_epilogue(const OpData<R> &op, const DslashArgs<R> &a, int p, unsigned cb, unsigned j)
+{
+    constexpr int NV = Vec<R>::NV;
+    if (XMODE != XM_NONE) {
+        const typename Vec<R>::T *q = a.xin + lb_index(j, 0, NV);
+#pragma unroll
+        for (int k = 0; k < NV; k++) prefetch_l1(q + 32 * k);
+    }
+    if (DOT == DOT_W) {
+        const typename Vec<R>::T *q = a.w + lb_index(j, 0, NV);
+#pragma unroll
+        for (int k = 0; k < NV; k++) prefetch_l1(q + 32 * k);
+    }
+    // clover rows are 16 bytes per lane in both precisions (float4 = two complex, double2 = one complex)
+    constexpr int ROWS = (sizeof(R) == 4) ? 18 : 36;
+    if (XMODE == XM_CLOVER) {
+        const char *q = reinterpret_cast<const char *>(p ? op.clov[1] : op.clov[0]) + ((size_t)(cb >> 5) * ROWS * 32 + (cb & 31u)) * 16;
+#pragma unroll
+        for (int k = 0; k < ROWS; k++) prefetch_l1(q + 512 * k);
+    }
+    if (PINV) {
+        const char *q = reinterpret_cast<const char *>(p ? op.clov_inv[1] : op.clov_inv[0]) + ((size_t)(cb >> 5) * ROWS * 32 + (cb & 31u)) * 16;
+#pragma unroll
+        for (int k = 0; k < ROWS; k++) prefetch_l1(q + 512 * k);
+    }
+}
+
 template <typename R, int B, int RECON, int XMODE, int PINV, int DOT>
 __global__ void __launch_bounds__(DSLASH_BLOCK, CLV_DSLASH_MINB) dslash_kernel(const Geom g, const OpData<R> op, const DslashArgs<R> a)
 {
@@ -164,17 +324,38 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, CLV_DSLASH_MINB) dslash_kernel(c
     if (active) {
         const int cb = j / B, rhs = j % B, p = a.parity;
         const Coord c = decode(g, cb, p);
+        HopAcc<R> hacc;
+        hacc.zero();
+        prefetch_epilogue<R, XMODE, PINV, DOT>(op, a, p, cb, j);
+        // fp32: loads of direction d+1 are issued before the arithmetic of direction d (measured best with 128 registers);
+        // fp64 has no registers to spare for that and runs the directions one after the other.
+        if constexpr (sizeof(R) == 4 && CLV_PIPE) {
+        HopIn<R> hin0, hin1;
+        hop_load<R, B, RECON, 0, 1>(g, op, a.in, p, cb, rhs, c, hin0);
+        hop_load<R, B, RECON, 0, 0>(g, op, a.in, p, cb, rhs, c, hin1);
+        hop_compute<R, RECON, 0, 1>(hin0, hacc);
+        hop_load<R, B, RECON, 1, 1>(g, op, a.in, p, cb, rhs, c, hin0);
+        hop_compute<R, RECON, 0, 0>(hin1, hacc);
+        hop_load<R, B, RECON, 1, 0>(g, op, a.in, p, cb, rhs, c, hin1);
+        hop_compute<R, RECON, 1, 1>(hin0, hacc);
+        hop_load<R, B, RECON, 2, 1>(g, op, a.in, p, cb, rhs, c, hin0);
+        hop_compute<R, RECON, 1, 0>(hin1, hacc);
+        hop_load<R, B, RECON, 2, 0>(g, op, a.in, p, cb, rhs, c, hin1);
+        hop_compute<R, RECON, 2, 1>(hin0, hacc);
+        hop_load<R, B, RECON, 3, 1>(g, op, a.in, p, cb, rhs, c, hin0);
+        hop_compute<R, RECON, 2, 0>(hin1, hacc);
+        hop_load<R, B, RECON, 3, 0>(g, op, a.in, p, cb, rhs, c, hin1);
+        hop_compute<R, RECON, 3, 1>(hin0, hacc);
+        hop_compute<R, RECON, 3, 0>(hin1, hacc);
+        } else
+        {
+            HopIn<R> d;
+#define CLV_HOP(MU, FW) hop_load<R, B, RECON, MU, FW>(g, op, a.in, p, cb, rhs, c, d); hop_compute<R, RECON, MU, FW>(d, hacc);
+            CLV_HOP(0, 1) CLV_HOP(0, 0) CLV_HOP(1, 1) CLV_HOP(1, 0) CLV_HOP(2, 1) CLV_HOP(2, 0) CLV_HOP(3, 1) CLV_HOP(3, 0)
+#undef CLV_HOP
+        }
         cx<R> acc[12];
-#pragma unroll
-        for (int i = 0; i < 12; i++) acc[i] = mk<R>(0, 0);
-        hop_dir<R, B, RECON, 0, 1>(g, op, a.in, p, cb, rhs, c, acc);
-        hop_dir<R, B, RECON, 0, 0>(g, op, a.in, p, cb, rhs, c, acc);
-        hop_dir<R, B, RECON, 1, 1>(g, op, a.in, p, cb, rhs, c, acc);
-        hop_dir<R, B, RECON, 1, 0>(g, op, a.in, p, cb, rhs, c, acc);
-        hop_dir<R, B, RECON, 2, 1>(g, op, a.in, p, cb, rhs, c, acc);
-        hop_dir<R, B, RECON, 2, 0>(g, op, a.in, p, cb, rhs, c, acc);
-        hop_dir<R, B, RECON, 3, 1>(g, op, a.in, p, cb, rhs, c, acc);
-        hop_dir<R, B, RECON, 3, 0>(g, op, a.in, p, cb, rhs, c, acc);
+        hacc.finish(acc);
 #pragma unroll
         for (int i = 0; i < 12; i++) acc[i] = a.coef * acc[i];
         cx<R> x[12];

@@ -51,7 +51,7 @@ __global__ void reorder_gauge_kernel(Geom g, const double *__restrict__ gauge, O
 #pragma unroll
     for (int k = 0; k < 9; k++) o64.gauge[p][mu][lb_index(cb, k, 9)] = make_double2(u[k].re, u[k].im);
 #pragma unroll
-    for (int k = 0; k < RECON32 / 2; k++) o32.gauge[p][mu][lb_index(cb, k, RECON32 / 2)] = make_float2((float)u[k].re, (float)u[k].im);
+    for (int k = 0; k < RECON32 / 2; k++) o32.gauge[p][mu][cplx_index<float>(cb, k, RECON32 / 2)] = make_float2((float)u[k].re, (float)u[k].im);
 }
 
 // ---- S1: clover term ------------------------------------------------------------------------------
@@ -188,7 +188,7 @@ __device__ void pack_block(const zc M[6][6], int blk, unsigned cb, double2 *o64,
     for (int k = 0; k < 3; k++) {
         const double a = M[2 * k][2 * k].re, b = M[2 * k + 1][2 * k + 1].re;
         o64[lb_index(cb, 18 * blk + k, 36)] = make_double2(a, b);
-        o32[lb_index(cb, 18 * blk + k, 36)] = make_float2((float)a, (float)b);
+        o32[cplx_index<float>(cb, 18 * blk + k, 36)] = make_float2((float)a, (float)b);
     }
     int k = 3;
     for (int i = 1; i < 6; i++)
@@ -196,7 +196,7 @@ __device__ void pack_block(const zc M[6][6], int blk, unsigned cb, double2 *o64,
             // Hermitian average of the two triangles (they agree to rounding)
             const double re = 0.5 * (M[i][j].re + M[j][i].re), im = 0.5 * (M[i][j].im - M[j][i].im);
             o64[lb_index(cb, 18 * blk + k, 36)] = make_double2(re, im);
-            o32[lb_index(cb, 18 * blk + k, 36)] = make_float2((float)re, (float)im);
+            o32[cplx_index<float>(cb, 18 * blk + k, 36)] = make_float2((float)re, (float)im);
         }
 }
 

@@ -19,6 +19,8 @@ struct SolveWork {
     void *sl[8] = {};          // x, r, p, v, s, t, r0, tmp  (float4 or double2 fields)
     double *partial = nullptr;
     int partial_blocks = 0;
+    double *stage = nullptr;
+    unsigned *ticket = nullptr;
     RhsScalars *sc_dev = nullptr, *sc_host = nullptr;
     double *stage_in = nullptr, *stage_out = nullptr;  // canonical staging for host-buffer solves
     size_t stage_bytes = 0;
@@ -37,6 +39,8 @@ void free_work(clover_ctx *ctx)
     if (!W) return;
     for (int i = 0; i < 8; i++) { cudaFree(W->f64[i]); cudaFree(W->sl[i]); }
     cudaFree(W->partial);
+    cudaFree(W->stage);
+    cudaFree(W->ticket);
     cudaFree(W->sc_dev);
     cudaFreeHost(W->sc_host);
     cudaFree(W->stage_in);
@@ -68,6 +72,9 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
             CLV_CUDA(cudaMalloc(&W->sc_dev, 8 * sizeof(RhsScalars)));
             CLV_CUDA(cudaMemset(W->sc_dev, 0, 8 * sizeof(RhsScalars)));
             CLV_CUDA(cudaMallocHost(&W->sc_host, 8 * sizeof(RhsScalars)));
+            CLV_CUDA(cudaMalloc(&W->stage, 8 * 32 * 4 * sizeof(double)));
+            CLV_CUDA(cudaMalloc(&W->ticket, 8 * sizeof(unsigned)));
+            CLV_CUDA(cudaMemset(W->ticket, 0, 8 * sizeof(unsigned)));
         }
         W->B_cap = B;
         W->sloppy_bytes = 0;
@@ -150,7 +157,7 @@ static double reliable_delta()
 {
     const char *e = getenv("CLOVER_DELTA");  // tuning/debug knob only
     const double d = e ? atof(e) : 0.0;
-    return (d > 0.0 && d < 1.0) ? d : 0.01;
+    return (d > 0.0 && d < 1.0) ? d : 1e-3;
 }
 
 template <typename R>
@@ -164,7 +171,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     V *x = (V *)W->sl[S_X], *r = (V *)W->sl[S_R], *p = (V *)W->sl[S_P], *v = (V *)W->sl[S_V], *s = (V *)W->sl[S_S], *t = (V *)W->sl[S_T],
       *r0 = (V *)W->sl[S_R0], *tmp = (V *)W->sl[S_TMP];
     long long &nl = ctx->stats.kernel_launches;
-    BlasCtx bc{&g, B, W->sc_dev, W->partial, W->partial_blocks, st, &nl};
+    BlasCtx bc{&g, B, W->sc_dev, W->partial, W->partial_blocks, W->stage, W->ticket, st, &nl};
     const double tol2 = tol * tol, delta = reliable_delta(), delta2 = delta * delta;
     const size_t nbytes = field_vecs<R>(g, B) * sizeof(V), nbytes64 = field_vecs<double>(g, B) * sizeof(double2);
     int nb = 0, grid = 0, iters = 0, updates = 0;
@@ -191,7 +198,21 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     CLV_CHECK(fetch_scalars(W, B, st));
 
     auto all_done = [&]() { for (int i = 0; i < B; i++) if (!W->sc_host[i].done) return false; return true; };
-    auto any_update = [&]() { for (int i = 0; i < B; i++) if (!W->sc_host[i].done && W->sc_host[i].want_update) return true; return false; };
+    // reliable update when any active rhs asks for one (delta rule), or when every active rhs claims convergence; a claim
+    // that has waited 3 iterations for the others is confirmed anyway
+    int claim_age = 0;
+    auto any_update = [&]() {
+        bool any_want = false, any_claim = false, all_claim = true;
+        for (int i = 0; i < B; i++) {
+            const RhsScalars &q = W->sc_host[i];
+            if (q.done) continue;
+            any_want |= q.want_update != 0;
+            any_claim |= q.claim != 0;
+            all_claim &= q.claim != 0;
+        }
+        claim_age = any_claim ? claim_age + 1 : 0;
+        return any_want || all_claim || claim_age >= 3;
+    };
     double ms_reliable = 0;
     while (!all_done() && iters < max_iter) {
         CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_W, r0, W->partial, &grid, st, W->kev));
@@ -221,6 +242,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[4], W->ev[5]));
             ms_reliable += ms;
             updates++;
+            claim_age = 0;
         }
         if (all_done()) break;
         CLV_CHECK(blas_p_update<R>(bc, p, r, v));
