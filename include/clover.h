@@ -90,8 +90,10 @@ int dslash_apply(clover_ctx *ctx, int op, int precision, const void *in_dev, voi
 int clover_solve(clover_ctx *ctx, const double *sources_dev, double *propagators_dev, int n_rhs, double tol,
                  int max_iter, int batch, int mixed, clover_rhs_info *info_host, void *stream);
 
-/* Same, end to end from HOST buffers: each batch is copied host -> device, solved, and its
- * propagators copied device -> host, all on `stream` (used for the e2e measurement). */
+/* Same, end to end from HOST buffers (pinned for full speed): batch i+1 is copied host -> device and the propagators of
+ * batch i-1 device -> host on two internal copy streams while batch i is solved on `stream` (double-buffered device
+ * staging owned by the context).  Work queued on `stream` before the call is waited for first; the call returns when
+ * every propagator is in propagators_host.  At most 64 batches per call.  (Used for the e2e measurement.) */
 int clover_solve_host(clover_ctx *ctx, const double *sources_host, double *propagators_host, int n_rhs, double tol,
                       int max_iter, int batch, int mixed, clover_rhs_info *info_host, void *stream);
 

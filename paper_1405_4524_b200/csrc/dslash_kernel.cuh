@@ -19,6 +19,9 @@ namespace clv {
 #ifndef CLV_DSLASH_MINB
 #define CLV_DSLASH_MINB 4 // <= 128 registers: measured best (ptxas keeps more loads in flight than with no hint; profiles/r1_tuning.md)
 #endif
+#ifndef CLV_DSLASH_MINB64
+#define CLV_DSLASH_MINB64 2
+#endif
 constexpr int DSLASH_BLOCK = CLV_DSLASH_BLOCK;
 
 template <typename R, int MU, int FWD> __device__ __forceinline__ void project(const cx<R> psi[12], cx<R> h[6])
@@ -286,6 +289,9 @@ template <int B, int BLOCK> __device__ __forceinline__ void block_reduce_rhs(dou
 #ifndef CLV_PIPE
 #define CLV_PIPE 1
 #endif
+#ifndef CLV_PIPE64
+#define CLV_PIPE64 0
+#endif
 __device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 template <typename R, int XMODE, int PINV, int DOT>
 __device__ __forceinline__ void prefetch_epilogue(const OpData<R> &op, const DslashArgs<R> &a, int p, unsigned cb, unsigned j)
@@ -316,7 +322,7 @@ __device__ __forceinline__ void prefetch_epilogue(const OpData<R> &op, const Dsl
 }
 
 template <typename R, int B, int RECON, int XMODE, int PINV, int DOT>
-__global__ void __launch_bounds__(DSLASH_BLOCK, CLV_DSLASH_MINB) dslash_kernel(const Geom g, const OpData<R> op, const DslashArgs<R> a)
+__global__ void __launch_bounds__(DSLASH_BLOCK, (sizeof(R) == 8 ? CLV_DSLASH_MINB64 : CLV_DSLASH_MINB)) dslash_kernel(const Geom g, const OpData<R> op, const DslashArgs<R> a)
 {
     const unsigned j = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
     const bool active = j < (unsigned)g.Vh * B;
@@ -329,7 +335,7 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, CLV_DSLASH_MINB) dslash_kernel(c
         prefetch_epilogue<R, XMODE, PINV, DOT>(op, a, p, cb, j);
         // fp32: loads of direction d+1 are issued before the arithmetic of direction d (measured best with 128 registers);
         // fp64 has no registers to spare for that and runs the directions one after the other.
-        if constexpr (sizeof(R) == 4 && CLV_PIPE) {
+        if constexpr (sizeof(R) == 4 ? CLV_PIPE : CLV_PIPE64) {
         HopIn<R> hin0, hin1;
         hop_load<R, B, RECON, 0, 1>(g, op, a.in, p, cb, rhs, c, hin0);
         hop_load<R, B, RECON, 0, 0>(g, op, a.in, p, cb, rhs, c, hin1);

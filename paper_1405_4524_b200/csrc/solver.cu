@@ -22,8 +22,12 @@ struct SolveWork {
     double *stage = nullptr;
     unsigned *ticket = nullptr;
     RhsScalars *sc_dev = nullptr, *sc_host = nullptr;
-    double *stage_in = nullptr, *stage_out = nullptr;  // canonical staging for host-buffer solves
+    // host-buffer solves: double-buffered canonical staging, copies on their own streams so that the H2D of batch i+1 and the
+    // D2H of batch i-1 overlap the solve of batch i
+    double *stage_in[2] = {}, *stage_out[2] = {};
     size_t stage_bytes = 0;
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_in[2] = {}, ev_out[2] = {};
     void *flush = nullptr;
     cudaEvent_t ev[6] = {};
     cudaEvent_t kev[6] = {};   // per-launch timing of the two sloppy Mhat calls of an iteration: 2 x (start, mid, end)
@@ -43,8 +47,9 @@ void free_work(clover_ctx *ctx)
     cudaFree(W->ticket);
     cudaFree(W->sc_dev);
     cudaFreeHost(W->sc_host);
-    cudaFree(W->stage_in);
-    cudaFree(W->stage_out);
+    for (int k = 0; k < 2; k++) { cudaFree(W->stage_in[k]); cudaFree(W->stage_out[k]); if (W->ev_in[k]) cudaEventDestroy(W->ev_in[k]); if (W->ev_out[k]) cudaEventDestroy(W->ev_out[k]); }
+    if (W->s_in) cudaStreamDestroy(W->s_in);
+    if (W->s_out) cudaStreamDestroy(W->s_out);
     cudaFree(W->flush);
     if (W->have_ev) for (int i = 0; i < 6; i++) { cudaEventDestroy(W->ev[i]); cudaEventDestroy(W->kev[i]); }
     delete W;
@@ -92,12 +97,22 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
     if (staging) {
         const size_t sb = (size_t)2 * g.Vh * 24 * sizeof(double) * W->B_cap;
         if (sb > W->stage_bytes) {
-            cudaFree(W->stage_in);
-            cudaFree(W->stage_out);
-            W->stage_in = W->stage_out = nullptr;
-            CLV_CUDA(cudaMalloc(&W->stage_in, sb));
-            CLV_CUDA(cudaMalloc(&W->stage_out, sb));
+            for (int k = 0; k < 2; k++) {
+                cudaFree(W->stage_in[k]);
+                cudaFree(W->stage_out[k]);
+                W->stage_in[k] = W->stage_out[k] = nullptr;
+                CLV_CUDA(cudaMalloc(&W->stage_in[k], sb));
+                CLV_CUDA(cudaMalloc(&W->stage_out[k], sb));
+            }
             W->stage_bytes = sb;
+        }
+        if (!W->s_in) {
+            CLV_CUDA(cudaStreamCreateWithFlags(&W->s_in, cudaStreamNonBlocking));
+            CLV_CUDA(cudaStreamCreateWithFlags(&W->s_out, cudaStreamNonBlocking));
+            for (int k = 0; k < 2; k++) {
+                CLV_CUDA(cudaEventCreateWithFlags(&W->ev_in[k], cudaEventDisableTiming));
+                CLV_CUDA(cudaEventCreateWithFlags(&W->ev_out[k], cudaEventDisableTiming));
+            }
         }
     }
     if (!W->have_ev) {
@@ -301,26 +316,45 @@ int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, do
     memset(&ctx->stats, 0, sizeof ctx->stats);
     const size_t per_rhs = (size_t)2 * ctx->geom.Vh * 24;  // doubles per canonical spinor
     int bad = 0, lastB = -1;
-    for (int done = 0; done < n_rhs;) {
-        const int B = next_batch(n_rhs - done, batch);
+    if (!host_buffers) {
+        for (int done = 0; done < n_rhs;) {
+            const int B = next_batch(n_rhs - done, batch);
+            if (B != lastB) CLV_CHECK(clear_fields(W, ctx->geom, B, st));
+            lastB = B;
+            int rc = mixed ? solve_batch<float>(ctx, src + done * per_rhs, dst + done * per_rhs, B, tol, max_iter, info + done, st)
+                           : solve_batch<double>(ctx, src + done * per_rhs, dst + done * per_rhs, B, tol, max_iter, info + done, st);
+            if (rc < 0) return rc;
+            bad += rc;
+            done += B;
+        }
+        return bad;
+    }
+    // host buffers: software pipeline over batches.  solve_batch synchronises `st` before it returns, so when batch i
+    // starts, batch i-1 no longer reads stage_in[(i+1)&1] and its result sits complete in stage_out[(i-1)&1].
+    CLV_CUDA(cudaStreamSynchronize(st));  // everything the caller queued on `st` before this call has happened
+    int nb = 0, start[64], size[64];
+    for (int done = 0; done < n_rhs && nb < 64; done += size[nb - 1]) { start[nb] = done; size[nb] = next_batch(n_rhs - done, batch); nb++; }
+    if (nb == 64 && start[63] + size[63] < n_rhs) { set_error("clover_solve_host: more than 64 batches in one call"); return CLOVER_EINVAL; }
+    auto h2d = [&](int i) {
+        return cudaMemcpyAsync(W->stage_in[i & 1], src + start[i] * per_rhs, per_rhs * size[i] * sizeof(double), cudaMemcpyHostToDevice, W->s_in) ||
+               cudaEventRecord(W->ev_in[i & 1], W->s_in);
+    };
+    CLV_CUDA((cudaError_t)h2d(0));
+    for (int i = 0; i < nb; i++) {
+        const int B = size[i], k = i & 1;
+        if (i + 1 < nb) CLV_CUDA((cudaError_t)h2d(i + 1));
         if (B != lastB) CLV_CHECK(clear_fields(W, ctx->geom, B, st));
         lastB = B;
-        const double *s = src + done * per_rhs;
-        double *d = dst + done * per_rhs;
-        if (host_buffers) {
-            CLV_CUDA(cudaMemcpyAsync(W->stage_in, s, per_rhs * B * sizeof(double), cudaMemcpyHostToDevice, st));
-            s = W->stage_in;
-            d = W->stage_out;
-        }
-        int rc = mixed ? solve_batch<float>(ctx, s, d, B, tol, max_iter, info + done, st) : solve_batch<double>(ctx, s, d, B, tol, max_iter, info + done, st);
+        CLV_CUDA(cudaStreamWaitEvent(st, W->ev_in[k], 0));
+        if (i >= 2) CLV_CUDA(cudaStreamWaitEvent(st, W->ev_out[k], 0));  // D2H of batch i-2 has drained stage_out[k]
+        int rc = mixed ? solve_batch<float>(ctx, W->stage_in[k], W->stage_out[k], B, tol, max_iter, info + start[i], st)
+                       : solve_batch<double>(ctx, W->stage_in[k], W->stage_out[k], B, tol, max_iter, info + start[i], st);
         if (rc < 0) return rc;
         bad += rc;
-        if (host_buffers) {
-            CLV_CUDA(cudaMemcpyAsync(dst + done * per_rhs, W->stage_out, per_rhs * B * sizeof(double), cudaMemcpyDeviceToHost, st));
-            CLV_CUDA(cudaStreamSynchronize(st));
-        }
-        done += B;
+        CLV_CUDA(cudaMemcpyAsync(dst + start[i] * per_rhs, W->stage_out[k], per_rhs * B * sizeof(double), cudaMemcpyDeviceToHost, W->s_out));
+        CLV_CUDA(cudaEventRecord(W->ev_out[k], W->s_out));
     }
+    CLV_CUDA(cudaStreamSynchronize(W->s_out));
     return bad;
 }
 
