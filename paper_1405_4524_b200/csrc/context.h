@@ -58,13 +58,14 @@ int reorder_out(const Geom &g, CT *canon, const typename Vec<R>::T *even, const 
 // ---- dslash.cu ----
 // out = P ( X + coef * H_{p,1-p} in ),  P = 1 | A_pp^-1,  X = 0 | xin | A_pp xin   (p = parity of out)
 enum { XM_NONE = 0, XM_PLAIN = 1, XM_CLOVER = 2 };
-enum { DOT_NONE = 0, DOT_W = 1, DOT_X = 2 };
+enum { DOT_NONE = 0, DOT_W = 1, DOT_X = 2, DOT_RES = 3 };
 template <typename R> struct DslashArgs {
     typedef typename Vec<R>::T V;
     const V *in;      // parity 1-p field
     const V *xin;     // parity p field (XM_PLAIN / XM_CLOVER)
     V *out;           // parity p field
-    const V *w;       // DOT_W: partial <w, out> per rhs
+    const V *w;       // DOT_W: partial <w, out> per rhs.  DOT_RES: the result is w - (...), partial ||result||^2
+    float4 *out32;    // DOT_RES only: if non-null the result is stored here in fp32 instead of `out` (reliable update: r = b - Mhat y)
     double *partial;  // [gridDim.x][B][4] : DOT_W -> (re,im of <w,out>, 0, 0); DOT_X -> (re,im of <out,xin>, <out,out>, 0)
     R coef;
     int parity;       // p

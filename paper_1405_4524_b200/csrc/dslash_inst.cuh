@@ -25,6 +25,7 @@ static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const Ds
         CLV_LAUNCH(XM_CLOVER, 0, DOT_NONE)
         CLV_LAUNCH(XM_CLOVER, 0, DOT_W)
         CLV_LAUNCH(XM_CLOVER, 0, DOT_X)
+        CLV_LAUNCH(XM_CLOVER, 0, DOT_RES)
     default:
         set_error("dslash: unsupported variant xmode=%d pinv=%d dot=%d", a.xmode, a.pinv, a.dot);
         return CLOVER_EINVAL;

@@ -302,7 +302,7 @@ __device__ __forceinline__ void prefetch_epilogue(const OpData<R> &op, const Dsl
 #pragma unroll
         for (int k = 0; k < NV; k++) prefetch_l1(q + 32 * k);
     }
-    if (DOT == DOT_W) {
+    if (DOT == DOT_W || DOT == DOT_RES) {
         const typename Vec<R>::T *q = a.w + lb_index(j, 0, NV);
 #pragma unroll
         for (int k = 0; k < NV; k++) prefetch_l1(q + 32 * k);
@@ -377,7 +377,21 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, (sizeof(R) == 8 ? CLV_DSLASH_MIN
 #pragma unroll
             for (int i = 0; i < 12; i++) acc[i] = t[i];
         }
-        store_spinor(a.out, j, acc);
+        if (DOT == DOT_RES) {  // residual epilogue: result = w - acc, ||result||^2, stored in the iteration precision
+            cx<R> w[12];
+            load_spinor(a.w, j, w);
+#pragma unroll
+            for (int i = 0; i < 12; i++) {
+                acc[i] = w[i] - acc[i];
+                d0 += (double)acc[i].re * (double)acc[i].re + (double)acc[i].im * (double)acc[i].im;
+            }
+            if (a.out32) {
+                cx<float> f[12];
+#pragma unroll
+                for (int i = 0; i < 12; i++) f[i] = mk<float>((float)acc[i].re, (float)acc[i].im);
+                store_spinor(a.out32, j, f);
+            } else store_spinor(a.out, j, acc);
+        } else store_spinor(a.out, j, acc);
         if (DOT == DOT_W) {
             cx<R> w[12];
             load_spinor(a.w, j, w);

@@ -141,7 +141,7 @@ template <typename R> static DslashArgs<R> dargs(const typename Vec<R>::T *in, c
                                                 int xmode, int pinv, int dot = DOT_NONE, const typename Vec<R>::T *w = nullptr, double *partial = nullptr)
 {
     DslashArgs<R> a;
-    a.in = in; a.xin = xin; a.out = out; a.w = w; a.partial = partial; a.coef = coef; a.parity = parity;
+    a.in = in; a.xin = xin; a.out = out; a.w = w; a.out32 = nullptr; a.partial = partial; a.coef = coef; a.parity = parity;
     a.xmode = xmode; a.pinv = pinv; a.dot = dot;
     return a;
 }
@@ -149,13 +149,15 @@ template <typename R> static DslashArgs<R> dargs(const typename Vec<R>::T *in, c
 // out_e = Mhat in_e, optional fused dot products; tmp is an odd-parity scratch field
 template <typename R>
 static int mhat(clover_ctx *ctx, int B, const typename Vec<R>::T *in, typename Vec<R>::T *tmp, typename Vec<R>::T *out, int dot, const typename Vec<R>::T *w,
-                double *partial, int *grid, cudaStream_t st, cudaEvent_t *kev = nullptr)
+                double *partial, int *grid, cudaStream_t st, cudaEvent_t *kev = nullptr, float4 *out32 = nullptr)
 {
     const R k2 = (R)(-ctx->kappa * ctx->kappa);
     if (kev) CLV_CUDA(cudaEventRecord(kev[0], st));
     CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(in, nullptr, tmp, (R)1, 1, XM_NONE, 1), B, st, nullptr));
     if (kev) CLV_CUDA(cudaEventRecord(kev[1], st));
-    CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(tmp, in, out, k2, 0, XM_CLOVER, 0, dot, w, partial), B, st, grid));
+    DslashArgs<R> a2 = dargs<R>(tmp, in, out, k2, 0, XM_CLOVER, 0, dot, w, partial);
+    a2.out32 = out32;
+    CLV_CHECK(launch_dslash<R>(ctx, a2, B, st, grid));
     if (kev) CLV_CUDA(cudaEventRecord(kev[2], st));
     ctx->stats.kernel_launches += 2;
     return 0;
@@ -249,9 +251,10 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             // reliable update: y += x, x = 0, r = b - Mhat y in fp64 (S 8(c) O6')
             CLV_CUDA(cudaEventRecord(W->ev[4], st));
             CLV_CHECK(blas_accumulate_y<R>(bc, y, x));
-            CLV_CHECK(mhat<double>(ctx, B, y, tmp64, w64, DOT_NONE, nullptr, nullptr, nullptr, st));
-            CLV_CHECK(blas_residual<R>(bc, b, w64, r64, r, &nb));
-            CLV_CHECK(blas_scalar_step(bc, SC_TRUE, nb, tol2, delta2));
+            // r = b - Mhat y with ||r||^2, fused into the epilogue of the second fp64 Dslash and stored in the iteration precision
+            CLV_CHECK(mhat<double>(ctx, B, y, tmp64, sizeof(R) == 8 ? (double2 *)r : nullptr, DOT_RES, b, W->partial, &grid, st, nullptr,
+                                   sizeof(R) == 4 ? (float4 *)r : nullptr));
+            CLV_CHECK(blas_scalar_step(bc, SC_TRUE, grid, tol2, delta2));
             CLV_CUDA(cudaEventRecord(W->ev[5], st));
             CLV_CHECK(fetch_scalars(W, B, st));
             CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[4], W->ev[5]));
