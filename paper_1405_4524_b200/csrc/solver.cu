@@ -32,6 +32,12 @@ struct SolveWork {
     cudaEvent_t ev[6] = {};
     cudaEvent_t kev[6] = {};   // per-launch timing of the two sloppy Mhat calls of an iteration: 2 x (start, mid, end)
     bool have_ev = false;
+    // launch-bound lattices: one iteration (10 kernels + the flag read-back) replayed as a CUDA graph on an internal stream
+    cudaStream_t s_work = nullptr;
+    cudaEvent_t ev_dep = nullptr;
+    cudaGraphExec_t iter_graph = nullptr;
+    int graph_B = 0, graph_prec = 0, graph_kernels = 0;
+    double graph_tol2 = 0, graph_delta2 = 0;
 };
 
 enum { F_ETA_E = 0, F_ETA_O, F_B, F_Y, F_R64, F_W64, F_TMP64, F_PSI_O };
@@ -52,6 +58,9 @@ void free_work(clover_ctx *ctx)
     if (W->s_out) cudaStreamDestroy(W->s_out);
     cudaFree(W->flush);
     if (W->have_ev) for (int i = 0; i < 6; i++) { cudaEventDestroy(W->ev[i]); cudaEventDestroy(W->kev[i]); }
+    if (W->iter_graph) cudaGraphExecDestroy(W->iter_graph);
+    if (W->s_work) cudaStreamDestroy(W->s_work);
+    if (W->ev_dep) cudaEventDestroy(W->ev_dep);
     delete W;
     ctx->work = nullptr;
 }
@@ -83,6 +92,7 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
         }
         W->B_cap = B;
         W->sloppy_bytes = 0;
+        if (W->iter_graph) { cudaGraphExecDestroy(W->iter_graph); W->iter_graph = nullptr; }
     }
     const size_t need = field_vecs<double>(g, W->B_cap) * 16 / 8 * real_bytes;  // float fields are half the size of double ones
     if (need > W->sloppy_bytes) {
@@ -93,6 +103,7 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
             CLV_CUDA(cudaMemset(W->sl[i], 0, need));
         }
         W->sloppy_bytes = need;
+        if (W->iter_graph) { cudaGraphExecDestroy(W->iter_graph); W->iter_graph = nullptr; }
     }
     if (staging) {
         const size_t sb = (size_t)2 * g.Vh * 24 * sizeof(double) * W->B_cap;
@@ -117,6 +128,8 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
     }
     if (!W->have_ev) {
         for (int i = 0; i < 6; i++) { CLV_CUDA(cudaEventCreate(&W->ev[i])); CLV_CUDA(cudaEventCreate(&W->kev[i])); }
+        CLV_CUDA(cudaStreamCreateWithFlags(&W->s_work, cudaStreamNonBlocking));
+        CLV_CUDA(cudaEventCreateWithFlags(&W->ev_dep, cudaEventDisableTiming));
         W->have_ev = true;
     }
     CLV_CUDA(cudaDeviceSynchronize());  // the memsets above ran on the legacy stream
@@ -177,12 +190,27 @@ static double reliable_delta()
     return (d > 0.0 && d < 1.0) ? d : 1e-3;
 }
 
+// Small lattices are launch-bound (a 16^3x32 Dslash takes ~10 us): replay the iteration as a CUDA graph there.
+static bool graph_enabled(const Geom &g, int B)
+{
+    const char *e = getenv("CLOVER_GRAPH");  // tuning/debug knob only
+    if (e) return atoi(e) != 0;
+    return (size_t)g.Vh * B * 96 < ((size_t)64 << 20);
+}
+
 template <typename R>
-static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, double tol, int max_iter, clover_rhs_info *info, cudaStream_t st)
+static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, double tol, int max_iter, clover_rhs_info *info, cudaStream_t st_user)
 {
     typedef typename Vec<R>::T V;
     SolveWork *W = ctx->work;
     const Geom &g = ctx->geom;
+    const bool use_graph = graph_enabled(g, B);
+    cudaStream_t st = st_user;
+    if (use_graph) {  // the legacy default stream cannot be captured: run on the internal stream, ordered after the caller's work
+        st = W->s_work;
+        CLV_CUDA(cudaEventRecord(W->ev_dep, st_user));
+        CLV_CUDA(cudaStreamWaitEvent(st, W->ev_dep, 0));
+    }
     double2 *eta_e = W->f64[F_ETA_E], *eta_o = W->f64[F_ETA_O], *b = W->f64[F_B], *y = W->f64[F_Y], *r64 = W->f64[F_R64], *w64 = W->f64[F_W64],
             *tmp64 = W->f64[F_TMP64], *psi_o = W->f64[F_PSI_O];
     V *x = (V *)W->sl[S_X], *r = (V *)W->sl[S_R], *p = (V *)W->sl[S_P], *v = (V *)W->sl[S_V], *s = (V *)W->sl[S_S], *t = (V *)W->sl[S_T],
@@ -231,22 +259,55 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         return any_want || all_claim || claim_age >= 3;
     };
     double ms_reliable = 0;
-    while (!all_done() && iters < max_iter) {
-        CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_W, r0, W->partial, &grid, st, W->kev));
+    // one BiCGStab iteration: [p update] Mhat p, alpha, s, Mhat s, omega, x/r update, rho/beta/flags, flag read-back
+    auto iteration = [&](bool with_p, cudaEvent_t *kev) -> int {
+        if (with_p) CLV_CHECK(blas_p_update<R>(bc, p, r, v));
+        CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_W, r0, W->partial, &grid, st, kev));
         CLV_CHECK(blas_scalar_step(bc, SC_ALPHA, grid, tol2, delta2));
         CLV_CHECK(blas_s_update<R>(bc, r, v, s));
-        CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_X, nullptr, W->partial, &grid, st, W->kev + 3));
+        CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_X, nullptr, W->partial, &grid, st, kev ? kev + 3 : nullptr));
         CLV_CHECK(blas_scalar_step(bc, SC_OMEGA, grid, tol2, delta2));
         CLV_CHECK(blas_xr_update<R>(bc, x, r, p, s, t, r0, &nb));
         CLV_CHECK(blas_scalar_step(bc, SC_RHO, nb, tol2, delta2));
-        CLV_CHECK(fetch_scalars(W, B, st));
-        iters++;
-        for (int h = 0; h < 2; h++) {
-            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h], W->kev[3 * h + 1])); ctx->stats.ms_ainv_hop += ms;
-            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h + 1], W->kev[3 * h + 2])); ctx->stats.ms_a_minus_hop += ms;
+        CLV_CUDA(cudaMemcpyAsync(W->sc_host, W->sc_dev, B * sizeof(RhsScalars), cudaMemcpyDeviceToHost, st));
+        return 0;
+    };
+    if (use_graph && (!W->iter_graph || W->graph_B != B || W->graph_prec != (int)sizeof(R) || W->graph_tol2 != tol2 || W->graph_delta2 != delta2)) {
+        if (W->iter_graph) { cudaGraphExecDestroy(W->iter_graph); W->iter_graph = nullptr; }
+        const long long nl0 = nl;
+        cudaGraph_t graph = nullptr;
+        CLV_CUDA(cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed));
+        const int rc = iteration(true, nullptr);
+        const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+        if (rc < 0) { if (graph) cudaGraphDestroy(graph); return rc; }
+        CLV_CUDA(ce);
+        W->graph_kernels = (int)(nl - nl0);
+        nl = nl0;  // capturing launched nothing
+        const cudaError_t ie = cudaGraphInstantiate(&W->iter_graph, graph, 0);
+        cudaGraphDestroy(graph);
+        CLV_CUDA(ie);
+        W->graph_B = B; W->graph_prec = (int)sizeof(R); W->graph_tol2 = tol2; W->graph_delta2 = delta2;
+    }
+    bool need_p = false;  // p = r before the first iteration
+    while (!all_done() && iters < max_iter) {
+        if (use_graph && need_p) {
+            CLV_CUDA(cudaGraphLaunch(W->iter_graph, st));
+            nl += W->graph_kernels;
+            CLV_CUDA(cudaStreamSynchronize(st));
+        } else {
+            CLV_CHECK(iteration(need_p, use_graph ? nullptr : W->kev));
+            CLV_CUDA(cudaStreamSynchronize(st));
+            if (!use_graph) {
+                for (int h = 0; h < 2; h++) {
+                    CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h], W->kev[3 * h + 1])); ctx->stats.ms_ainv_hop += ms;
+                    CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h + 1], W->kev[3 * h + 2])); ctx->stats.ms_a_minus_hop += ms;
+                }
+                ctx->stats.n_ainv_hop += 2;
+                ctx->stats.n_a_minus_hop += 2;
+            }
         }
-        ctx->stats.n_ainv_hop += 2;
-        ctx->stats.n_a_minus_hop += 2;
+        iters++;
+        need_p = true;
         if (any_update() || iters == max_iter) {
             // reliable update: y += x, x = 0, r = b - Mhat y in fp64 (S 8(c) O6')
             CLV_CUDA(cudaEventRecord(W->ev[4], st));
@@ -262,8 +323,6 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             updates++;
             claim_age = 0;
         }
-        if (all_done()) break;
-        CLV_CHECK(blas_p_update<R>(bc, p, r, v));
     }
     CLV_CUDA(cudaEventRecord(W->ev[3], st));
     // odd sites and verification on the full lattice, all fp64
