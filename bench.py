@@ -273,6 +273,26 @@ def main():
                "wall_s_per_step": (time.perf_counter() - t0) / args.steps}
         del h_eta, h_psi
 
+    # ---- NEXT row (S 8(f) rank 1): stochastic-operator contraction O_ij(t) of the step's sources and solutions ----
+    contraction = None
+    if rank == 0:
+        o = B.stochastic_operators(eta, psi)
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for _ in range(5):
+            o = B.stochastic_operators(eta, psi)
+        c1.record()
+        torch.cuda.synchronize()
+        tc = c0.elapsed_time(c1) / 5 * 1e-3
+        cbytes = 2 * n_rhs * V * 24 * 8
+        cflop = 8.0 * n_rhs * n_rhs * 12 * V
+        fp64_peak = 148 * 64 * 2 * 1.965e9     # fp64 FMA lanes per SM x SMs x 2 flop x max clock
+        contraction = {"what": "O_ij(t) = sum_y eta_i^* gamma5 X_j, all t, N_r = %d (paper eq. 7.6)" % n_rhs, "ms": tc * 1e3,
+                       "gbs": cbytes / tc / 1e9, "frac_hbm": cbytes / tc / 1e9 / peaks["hbm_gbs"], "tflops_fp64": cflop / tc / 1e12,
+                       "frac_fp64_alu": cflop / tc / fp64_peak, "bound": "alu (fp64 FMA) ~ hbm", "dtype": "f64"}
+        del o
+
     if rank != 0:
         return
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -282,7 +302,7 @@ def main():
                       "eps": cfg["eps"], "recon": cfg["recon"], "time_dilution": cfg["dilution"],
                       "solver": "even-odd BiCGStab, fp32 iteration + fp64 reliable updates" if cfg["mixed"] else "even-odd BiCGStab fp64",
                       "l2": "fields per sweep (>= 255 MB at batch 8) exceed the 126 MB L2; the stand-alone hop timing flushes L2 between launches"},
-           "clocks": sampler.summary(), "gpu_launches": launches, "roofline": roofline, "dslash": dslash, "e2e": e2e,
+           "clocks": sampler.summary(), "gpu_launches": launches, "roofline": roofline, "dslash": dslash, "e2e": e2e, "next_contraction": contraction,
            "solve": {"iters": [i["iters"] for i in last["infos"]][::batch], "reliable_updates": [i["reliable_updates"] for i in last["infos"]][::batch],
                      "max_true_resid": max(i["true_resid"] for i in last["infos"]),
                      "phase_ms_per_step": {k: v / args.steps for k, v in phases.items()}}}

@@ -103,6 +103,16 @@ int clover_solve_host(clover_ctx *ctx, const double *sources_host, double *propa
 int noise_fill(void *out_dev, int precision, const int dims[4], uint64_t seed, int n_rhs, int rhs_offset,
                int time_dilution, double scale, void *stream);
 
+/* ---- stochastic-operator contraction (S 8(f) rank 1; paper eqs. 7.5-7.7) ---- */
+/* O_ij(t) = sum_y eta_i^*(t,y) gamma5 X_j(t,y)  (eq. 7.6: sum over the timeslice, spin and colour; gamma5 = diag(+,+,-,-) in the
+ * basis R1).  eta_dev, x_dev: n_rhs canonical fp64 spinors each (device); o_dev: double [T][n_rhs][n_rhs][2] (device), index
+ * [t][i][j].  fp64 arithmetic, deterministic summation order.  Needs no context; scratch is stream-ordered
+ * (cudaMallocAsync).  Asynchronous on `stream`. */
+int stochastic_operators(const double *eta_dev, const double *x_dev, const int dims[4], int n_rhs, double *o_dev, void *stream);
+/* C(t0, t) = (1 / (n_rhs^2 scale^4)) sum_ij O_ij(t) O_ji(t0)  (eq. 7.7 for every pair of timeslices; scale = the noise scale,
+ * R7).  o_dev as above; c_dev: double [T][T][2] (device), index [t0][t].  Asynchronous on `stream`. */
+int stochastic_correlator(const double *o_dev, int T, int n_rhs, double scale, double *c_dev, void *stream);
+
 /* ---- measurement helpers (internal layout, no reorders; used by bench.py and the ncu runs) ---- */
 enum {
     CLOVER_KERNEL_HOP = 0,        /* out_e = H_eo in_o                          (1320 flop/site)  */

@@ -18,7 +18,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 OP_HOP_EO, OP_HOP_OE, OP_HOP_FULL, OP_CLOVER, OP_CLOVER_INV, OP_D_FULL, OP_MHAT = range(7)
 KERNEL_HOP, KERNEL_AINV_HOP, KERNEL_A_MINUS_HOP = range(3)
 EXPORTS = ["clover_create", "clover_destroy", "dslash_apply", "clover_solve", "clover_solve_host", "noise_fill",
-           "clover_bench_kernel", "clover_get_stats", "clover_last_error"]
+           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator"]
 
 
 class ClovOpts(ctypes.Structure):
@@ -48,6 +48,8 @@ _lib.noise_fill.argtypes = [_vp, _i, _ip, ctypes.c_uint64, _i, _i, _i, _d, _vp]
 _lib.clover_bench_kernel.argtypes = [_vp, _i, _i, _i, _i, _i, ctypes.POINTER(ctypes.c_float), _vp]
 _lib.clover_get_stats.argtypes = [_vp, ctypes.POINTER(SolveStats)]
 _lib.clover_last_error.argtypes = [_vp]
+_lib.stochastic_operators.argtypes = [_vp, _vp, _ip, _i, _vp, _vp]
+_lib.stochastic_correlator.argtypes = [_vp, _i, _i, _d, _vp, _vp]
 _lib.clover_last_error.restype = ctypes.c_char_p
 
 
@@ -88,6 +90,27 @@ def noise_fill(dims, seed, n_rhs, rhs_offset=0, time_dilution=0, scale=1.0, dtyp
     prec = 64 if out.dtype == torch.complex128 else 32
     _check(_lib.noise_fill(out.data_ptr(), prec, _i4(dims), seed, n_rhs, rhs_offset, int(time_dilution), float(scale), _stream()))
     return out
+
+
+def stochastic_operators(eta, x):
+    """O[t, i, j] = sum_y eta_i^*(t, y) gamma5 X_j(t, y) (paper eq. 7.6); eta, x complex128 [n, T, Z, Y, X, 4, 3] on the device."""
+    _require_cuda()
+    assert eta.is_cuda and x.is_cuda and eta.is_contiguous() and x.is_contiguous() and eta.dtype == x.dtype == torch.complex128
+    assert eta.shape == x.shape
+    n, T, Z, Y, X = eta.shape[:5]
+    o = torch.empty((T, n, n), dtype=torch.complex128, device="cuda")
+    _check(_lib.stochastic_operators(eta.data_ptr(), x.data_ptr(), _i4((X, Y, Z, T)), n, o.data_ptr(), _stream()))
+    return o
+
+
+def stochastic_correlator(o, scale=1.0):
+    """C[t0, t] = (1 / (n^2 scale^4)) sum_ij O[t, i, j] O[t0, j, i] (paper eq. 7.7)."""
+    _require_cuda()
+    assert o.is_cuda and o.is_contiguous() and o.dtype == torch.complex128 and o.shape[1] == o.shape[2]
+    T, n = o.shape[0], o.shape[1]
+    c = torch.empty((T, T), dtype=torch.complex128, device="cuda")
+    _check(_lib.stochastic_correlator(o.data_ptr(), T, n, float(scale), c.data_ptr(), _stream()))
+    return c
 
 
 class Clover:

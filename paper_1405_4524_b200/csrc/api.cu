@@ -117,6 +117,23 @@ int noise_fill(void *out_dev, int precision, const int dims[4], uint64_t seed, i
     return launch_noise(out_dev, precision, dims, seed, n_rhs, rhs_offset, time_dilution != 0, scale, (cudaStream_t)stream);
 }
 
+int stochastic_operators(const double *eta_dev, const double *x_dev, const int dims[4], int n_rhs, double *o_dev, void *stream)
+{
+    if (!eta_dev || !x_dev || !o_dev) { set_error("stochastic_operators: null argument"); return CLOVER_EINVAL; }
+    CLV_CHECK(check_dims(dims));
+    if (n_rhs < 1) { set_error("stochastic_operators: n_rhs = %d must be >= 1", n_rhs); return CLOVER_EINVAL; }
+    CLV_CHECK(check_device());
+    return launch_contract(eta_dev, x_dev, dims, n_rhs, o_dev, (cudaStream_t)stream);
+}
+
+int stochastic_correlator(const double *o_dev, int T, int n_rhs, double scale, double *c_dev, void *stream)
+{
+    if (!o_dev || !c_dev) { set_error("stochastic_correlator: null argument"); return CLOVER_EINVAL; }
+    if (T < 1 || n_rhs < 1 || !(scale > 0.0)) { set_error("stochastic_correlator: bad T, n_rhs or scale"); return CLOVER_EINVAL; }
+    CLV_CHECK(check_device());
+    return launch_correlator(o_dev, T, n_rhs, scale, c_dev, (cudaStream_t)stream);
+}
+
 int clover_bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms_per_launch, void *stream)
 {
     if (!ctx || !ms_per_launch) { set_error("clover_bench_kernel: null argument"); return CLOVER_EINVAL; }
