@@ -14,14 +14,21 @@ namespace clv {
 
 constexpr int CT_TILE = 32;    // (i, j) tile edge
 constexpr int CT_KT = 16;      // k elements staged per step
-constexpr int CT_THREADS = 64; // 8 x 8 threads, each a 4 x 4 block of outputs {ti + 8a} x {tj + 8b}
+constexpr int CT_THREADS = 64;  // 8 x 8 threads, each a 4 x 4 block of outputs {ti + 8a} x {tj + 8b}
+#ifndef CT_MINB
+#define CT_MINB 8
+#endif
+#ifndef CT_UNROLL
+#define CT_UNROLL 2
+#endif
+constexpr int CT_UNROLL_N = CT_UNROLL;
 
 // partial[(c*T + t)*n*n + i*n + j] = sum over k-chunk c of conj(eta_i[k]) g5(k) X_j[k]
 // Two-stage cp.async pipeline: the 16-byte copies of stage s+1 (global -> shared, no registers) are in flight while stage s
 // is multiplied.  Shared tiles are stored [row][k] with a row stride of 17 x 16 bytes: the copies are coalesced along k
 // (a half-warp moves 256 contiguous bytes of one row) and the compute-phase reads of 8 different rows at one k fall in 8
 // different bank groups (lanes sharing ti get a broadcast).  conj() and the gamma5 sign are applied when the tile is read back from shared memory.
-__global__ void __launch_bounds__(CT_THREADS, 6) contract_kernel(const double2 *__restrict__ eta, const double2 *__restrict__ xs, int n, int T,
+__global__ void __launch_bounds__(CT_THREADS, CT_MINB) contract_kernel(const double2 *__restrict__ eta, const double2 *__restrict__ xs, int n, int T,
                                                                  long K, long kchunk, int tiles, double2 *__restrict__ partial)
 {
     __shared__ __align__(16) double2 As[2][CT_TILE][CT_KT + 1], Bs[2][CT_TILE][CT_KT + 1];
@@ -58,7 +65,7 @@ __global__ void __launch_bounds__(CT_THREADS, 6) contract_kernel(const double2 *
             __pipeline_wait_prior(1);
         } else __pipeline_wait_prior(0);
         __syncthreads();
-#pragma unroll 4
+#pragma unroll CT_UNROLL_N
         for (int kk = 0; kk < CT_KT; kk++) {
             const double sgn = (((kb + kk) % 12) < 6) ? 1.0 : -1.0;   // gamma5 = diag(+,+,-,-), spin = (k % 12) / 3
             double2 a[4], b[4];
