@@ -98,10 +98,11 @@ int clover_solve_host(clover_ctx *ctx, const double *sources_host, double *propa
                       int max_iter, int batch, int mixed, clover_rhs_info *info_host, void *stream);
 
 /* Z4 noise sources (docs/NOISE.md): out_dev = n_rhs canonical spinors, precision 32 | 64,
- * source index r = rhs_offset + j; time_dilution = 1 keeps only timeslice t = r mod T.
+ * source index r = rhs_offset + j; dilution: bit 0 keeps only timeslice t = r mod T, bit 1 keeps only the spin-colour
+ * component (r / T, or r without the time bit) mod 12 ("time-spin-color dilution"); 0 = undiluted.
  * Needs no context.  Asynchronous on `stream`.  Bit-exact against the written spec. */
 int noise_fill(void *out_dev, int precision, const int dims[4], uint64_t seed, int n_rhs, int rhs_offset,
-               int time_dilution, double scale, void *stream);
+               int dilution, double scale, void *stream);
 
 /* ---- stochastic-operator contraction (S 8(f) rank 1; paper eqs. 7.5-7.7) ---- */
 /* O_ij(t) = sum_y eta_i^*(t,y) gamma5 X_j(t,y)  (eq. 7.6: sum over the timeslice, spin and colour; gamma5 = diag(+,+,-,-) in the

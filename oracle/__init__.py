@@ -151,9 +151,11 @@ def splitmix64(seed, ctr):
     return int(lib().oracle_splitmix64(ctypes.c_uint64(seed), ctypes.c_uint64(ctr)))
 
 
-def noise_fill(dims, seed, n_rhs, rhs_offset=0, time_dilution=0, scale=1.0, dtype=np.float64):
+def noise_fill(dims, seed, n_rhs, rhs_offset=0, time_dilution=0, scale=1.0, dtype=np.float64, dilution=None):
     """Z4 sources, SURVEY 8(c) O5 / docs/NOISE.md: complex [n_rhs, T, Z, Y, X, 4, 3]."""
     X, Y, Z, T = dims
+    if dilution is not None:      # bit 0 = time, bit 1 = spin-colour (docs/NOISE.md); time_dilution=1 is dilution=1
+        time_dilution = dilution
     if dtype == np.float64:
         out = np.empty((n_rhs, T, Z, Y, X, 4, 3), dtype=np.complex128)
         lib().oracle_noise_fill(_p(out), _i4(dims), ctypes.c_uint64(seed), ctypes.c_int(n_rhs),

@@ -419,6 +419,18 @@ uint64_t oracle_splitmix64(uint64_t seed, uint64_t ctr)
     return z ^ (z >> 31);
 }
 
+/* dilution (bit 0 = time, bit 1 = spin-colour; docs/NOISE.md): source r lives on timeslice t_r = r mod T (time bit) and on the
+ * single spin-colour component sc_r = (r / T) mod 12 (both bits) or r mod 12 (spin-colour only), sc = 3*spin + colour. */
+static int oracle_noise_keep(int dilution, uint64_t r, int t, int sc, int T)
+{
+    if ((dilution & 1) && t != (int)(r % (uint64_t)T)) return 0;
+    if (dilution & 2) {
+        const uint64_t q = (dilution & 1) ? r / (uint64_t)T : r;
+        if (sc != (int)(q % 12ULL)) return 0;
+    }
+    return 1;
+}
+
 void oracle_noise_fill(double *out, const int dims[4], uint64_t seed, int n_rhs, int rhs_offset,
                        int time_dilution, double scale)
 {
@@ -431,7 +443,7 @@ void oracle_noise_fill(double *out, const int dims[4], uint64_t seed, int n_rhs,
         for (long n = 0; n < V * 12; n++) {
             int t = (int)((n / 12) / ((long)dims[0] * dims[1] * dims[2]));
             int k = (int)(oracle_splitmix64(seed, r * 12ULL * (uint64_t)V + (uint64_t)n) >> 62);
-            if (time_dilution && t != (int)(r % (uint64_t)dims[3])) { o[2 * n] = 0.0; o[2 * n + 1] = 0.0; }
+            if (!oracle_noise_keep(time_dilution, r, t, (int)(n % 12), dims[3])) { o[2 * n] = 0.0; o[2 * n + 1] = 0.0; }
             else { o[2 * n] = tab[k][0]; o[2 * n + 1] = tab[k][1]; }
         }
     }
@@ -449,7 +461,7 @@ void oracle_noise_fill_f32(float *out, const int dims[4], uint64_t seed, int n_r
         for (long n = 0; n < V * 12; n++) {
             int t = (int)((n / 12) / ((long)dims[0] * dims[1] * dims[2]));
             int k = (int)(oracle_splitmix64(seed, r * 12ULL * (uint64_t)V + (uint64_t)n) >> 62);
-            if (time_dilution && t != (int)(r % (uint64_t)dims[3])) { o[2 * n] = 0.0f; o[2 * n + 1] = 0.0f; }
+            if (!oracle_noise_keep(time_dilution, r, t, (int)(n % 12), dims[3])) { o[2 * n] = 0.0f; o[2 * n + 1] = 0.0f; }
             else { o[2 * n] = tab[k][0]; o[2 * n + 1] = tab[k][1]; }
         }
     }

@@ -81,9 +81,11 @@ def _spinor_shape(dims, n_rhs):
     return (n_rhs, T, Z, Y, X, 4, 3)
 
 
-def noise_fill(dims, seed, n_rhs, rhs_offset=0, time_dilution=0, scale=1.0, dtype=torch.complex128, out=None):
+def noise_fill(dims, seed, n_rhs, rhs_offset=0, time_dilution=0, scale=1.0, dtype=torch.complex128, out=None, dilution=None):
     """Z4 noise sources on the device: complex [n_rhs, T, Z, Y, X, 4, 3] (include/clover.h: noise_fill)."""
     _require_cuda()
+    if dilution is not None:      # bit 0 = time, bit 1 = spin-colour; time_dilution=1 is dilution=1
+        time_dilution = dilution
     if out is None:
         out = torch.empty(_spinor_shape(dims, n_rhs), dtype=dtype, device="cuda")
     assert out.is_cuda and out.is_contiguous() and out.dtype in (torch.complex64, torch.complex128)

@@ -107,14 +107,15 @@ int clover_solve_host(clover_ctx *ctx, const double *sources_host, double *propa
     return solve_common(ctx, sources_host, propagators_host, n_rhs, tol, max_iter, batch, mixed, info_host, stream, 1);
 }
 
-int noise_fill(void *out_dev, int precision, const int dims[4], uint64_t seed, int n_rhs, int rhs_offset, int time_dilution, double scale, void *stream)
+int noise_fill(void *out_dev, int precision, const int dims[4], uint64_t seed, int n_rhs, int rhs_offset, int dilution, double scale, void *stream)
 {
     if (!out_dev) { set_error("noise_fill: null output"); return CLOVER_EINVAL; }
     CLV_CHECK(check_dims(dims));
     if (precision != 32 && precision != 64) { set_error("precision = %d must be 32 or 64", precision); return CLOVER_EINVAL; }
     if (n_rhs < 0 || rhs_offset < 0) { set_error("noise_fill: negative n_rhs or rhs_offset"); return CLOVER_EINVAL; }
     CLV_CHECK(check_device());
-    return launch_noise(out_dev, precision, dims, seed, n_rhs, rhs_offset, time_dilution != 0, scale, (cudaStream_t)stream);
+    if (dilution < 0 || dilution > 3) { set_error("noise_fill: dilution = %d must be 0..3 (bit 0 time, bit 1 spin-colour)", dilution); return CLOVER_EINVAL; }
+    return launch_noise(out_dev, precision, dims, seed, n_rhs, rhs_offset, dilution, scale, (cudaStream_t)stream);
 }
 
 int stochastic_operators(const double *eta_dev, const double *x_dev, const int dims[4], int n_rhs, double *o_dev, void *stream)

@@ -35,13 +35,13 @@ __global__ void __launch_bounds__(256) noise_kernel(R *__restrict__ out, uint64_
         const uint64_t j = i / pairs_per_rhs, n = 2 * (i % pairs_per_rhs);
         const uint64_t r = (uint64_t)rhs_offset + j;
         R v[4];
-        const bool keep = !dilution || (int)((n / 12) / sites_per_t) == (int)(r % (uint64_t)T);  // n and n+1 share a site
-        if (keep) {
-            z4_value<R>(z4_index(seed, r * n12V + n), scale, v[0], v[1]);
-            z4_value<R>(z4_index(seed, r * n12V + n + 1), scale, v[2], v[3]);
-        } else {
-            v[0] = v[1] = v[2] = v[3] = (R)0;
-        }
+        // dilution: bit 0 keeps timeslice r mod T only, bit 1 keeps spin-colour component (r / T or r) mod 12 only (docs/NOISE.md)
+        const bool keep_t = !(dilution & 1) || (int)((n / 12) / sites_per_t) == (int)(r % (uint64_t)T);  // n and n+1 share a site
+        const int sc_r = (dilution & 2) ? (int)(((dilution & 1) ? r / (uint64_t)T : r) % 12ULL) : -1;
+        const int sc0 = (int)(n % 12);
+        v[0] = v[1] = v[2] = v[3] = (R)0;
+        if (keep_t && (sc_r < 0 || sc_r == sc0)) z4_value<R>(z4_index(seed, r * n12V + n), scale, v[0], v[1]);
+        if (keep_t && (sc_r < 0 || sc_r == sc0 + 1)) z4_value<R>(z4_index(seed, r * n12V + n + 1), scale, v[2], v[3]);
         R *dst = out + (j * n12V + n) * 2;
         if (sizeof(R) == 4) {
             *reinterpret_cast<float4 *>(dst) = make_float4((float)v[0], (float)v[1], (float)v[2], (float)v[3]);

@@ -104,6 +104,13 @@ def test_noise_bit_exact(B, dims):
             want32 = oracle.noise_fill(dims, 2001, 3, rhs_offset=off, time_dilution=dil, scale=s, dtype=np.float32)
             got32 = B.noise_fill(dims, 2001, 3, rhs_offset=off, time_dilution=dil, scale=s, dtype=torch.complex64).cpu().numpy()
             assert np.array_equal(got32.view(np.uint32), want32.view(np.uint32))
+    for dil in (2, 3):      # spin-colour and time-spin-colour dilution
+        want = oracle.noise_fill(dims, 2004, 30, rhs_offset=7, dilution=dil, scale=s)
+        got = B.noise_fill(dims, 2004, 30, rhs_offset=7, dilution=dil, scale=s).cpu().numpy()
+        assert np.array_equal(got.view(np.uint64), want.view(np.uint64))
+        want32 = oracle.noise_fill(dims, 2004, 30, rhs_offset=7, dilution=dil, scale=s, dtype=np.float32)
+        got32 = B.noise_fill(dims, 2004, 30, rhs_offset=7, dilution=dil, scale=s, dtype=torch.complex64).cpu().numpy()
+        assert np.array_equal(got32.view(np.uint32), want32.view(np.uint32))
 
 
 def _check_solutions(S, eta, psi, infos, tol=1e-10, oracle_tol=1e-12, which=None):

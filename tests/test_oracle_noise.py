@@ -65,3 +65,28 @@ def test_noise_time_dilution_is_a_mask():
     a = oracle.noise_fill(dims, 7, 3, rhs_offset=0, scale=1.0)
     b = oracle.noise_fill(dims, 7, 1, rhs_offset=2, scale=1.0)
     assert np.array_equal(a[2], b[0])
+
+
+def test_spin_colour_dilution_masks_and_covers():
+    """dilution bits (docs/NOISE.md; "time-spin-color dilution"): each source is a masked copy of its undiluted
+    stream, and 12 T consecutive time-spin-colour diluted sources touch every (t, spin, colour) exactly once."""
+    dims = (2, 2, 2, 4)
+    T = 4
+    n = 12 * T
+    full = oracle.noise_fill(dims, 9, n, scale=1.0)
+    tsc = oracle.noise_fill(dims, 9, n, scale=1.0, dilution=3)
+    sc_only = oracle.noise_fill(dims, 9, 24, scale=1.0, dilution=2)
+    cover = np.zeros((T, 4, 3), dtype=int)
+    for r in range(n):
+        t_r, sc_r = r % T, (r // T) % 12
+        mask = np.zeros(full[r].shape, dtype=bool)
+        mask[t_r, :, :, :, sc_r // 3, sc_r % 3] = True
+        assert np.array_equal(tsc[r][mask], full[r][mask]) and np.all(tsc[r][~mask] == 0)
+        assert not np.signbit(tsc[r].real).any() or np.all(tsc[r].real[np.signbit(tsc[r].real)] != 0)
+        cover[t_r, sc_r // 3, sc_r % 3] += 1
+    assert np.all(cover == 1)
+    for r in range(24):
+        sc_r = r % 12
+        mask = np.zeros(full[r].shape, dtype=bool)
+        mask[:, :, :, :, sc_r // 3, sc_r % 3] = True
+        assert np.array_equal(sc_only[r][mask], full[r][mask]) and np.all(sc_only[r][~mask] == 0)
