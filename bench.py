@@ -293,6 +293,34 @@ def main():
                        "frac_fp64_alu": cflop / tc / fp64_peak, "bound": "alu (fp64 FMA) ~ hbm", "dtype": "f64"}
         del o
 
+    # ---- NEXT row (S 8(f) rank 2): outer-product fill S and S^dagger at the paper's Table II size (L = 8: 8^3x16) ----
+    fill_res = None
+    if rank == 0 and args.config == 3:
+        fd = (8, 8, 8, 16)
+        fe = B.noise_fill(fd, 2001, n_rhs, scale=wl.INV_SQRT2)
+        fx = B.noise_fill(fd, 977, n_rhs, scale=1.0)
+        fs = torch.empty((16, 512, 12, 512, 12), dtype=torch.complex128, device="cuda")
+        times = {}
+        for dag in (0, 1):
+            B.stochastic_fill(fx, fe, t0=0, scale=wl.INV_SQRT2, dagger=bool(dag), out=fs.view((512, 12, 16, 512, 12)) if dag else fs)
+            torch.cuda.synchronize()
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record()
+            for _ in range(3):
+                B.stochastic_fill(fx, fe, t0=0, scale=wl.INV_SQRT2, dagger=bool(dag), out=fs.view((512, 12, 16, 512, 12)) if dag else fs)
+            c1.record()
+            torch.cuda.synchronize()
+            times[dag] = c0.elapsed_time(c1) / 3 * 1e-3
+        fbytes = fs.numel() * 16
+        fflop = 8.0 * fs.numel() * n_rhs
+        fp64_peak = 148 * 64 * 2 * 1.965e9
+        fill_res = {"what": "S and S^dagger fill (paper eq. 7.3), 8^3x16, N_r = %d in one pass, 9.66 GB each" % n_rhs,
+                    "ms_fill": times[0] * 1e3, "ms_fill_dagger": times[1] * 1e3, "write_gbs": fbytes / times[0] / 1e9,
+                    "tflops_fp64": fflop / times[0] / 1e12, "frac_fp64_alu": fflop / times[0] / fp64_peak,
+                    "frac_hbm_write": fbytes / times[0] / 1e9 / peaks["hbm_gbs"], "ms_per_source_both": (times[0] + times[1]) * 1e3 / n_rhs,
+                    "paper_table2_s_per_source": {"cpu": 100.8, "gpu": 8.8, "hardware": "unnamed", "cite": "PAPER.md L340-344"}}
+        del fs, fe, fx
+
     if rank != 0:
         return
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -302,7 +330,7 @@ def main():
                       "eps": cfg["eps"], "recon": cfg["recon"], "time_dilution": cfg["dilution"],
                       "solver": "even-odd BiCGStab, fp32 iteration + fp64 reliable updates" if cfg["mixed"] else "even-odd BiCGStab fp64",
                       "l2": "fields per sweep (>= 255 MB at batch 8) exceed the 126 MB L2; the stand-alone hop timing flushes L2 between launches"},
-           "clocks": sampler.summary(), "gpu_launches": launches, "roofline": roofline, "dslash": dslash, "e2e": e2e, "next_contraction": contraction,
+           "clocks": sampler.summary(), "gpu_launches": launches, "roofline": roofline, "dslash": dslash, "e2e": e2e, "next_contraction": contraction, "next_fill": fill_res,
            "solve": {"iters": [i["iters"] for i in last["infos"]][::batch], "reliable_updates": [i["reliable_updates"] for i in last["infos"]][::batch],
                      "max_true_resid": max(i["true_resid"] for i in last["infos"]),
                      "phase_ms_per_step": {k: v / args.steps for k, v in phases.items()}}}

@@ -114,6 +114,15 @@ int stochastic_operators(const double *eta_dev, const double *x_dev, const int d
  * R7).  o_dev as above; c_dev: double [T][T][2] (device), index [t0][t].  Asynchronous on `stream`. */
 int stochastic_correlator(const double *o_dev, int T, int n_rhs, double scale, double *c_dev, void *stream);
 
+/* ---- outer-product fill (S 8(f) rank 2; paper eq. 7.3, Tables I-II "S_s fill", "S_s^dagger fill") ---- */
+/* S(t,z,a; t0,x,b) = (1/(n_rhs scale^2)) sum_i X_i(t,z,a) conj(eta_i(t0,x,b)),  a, b = 3*spin + colour, z and x spatial sites in
+ * canonical (z,y,x) order.  x_dev, eta_dev: n_rhs canonical fp64 spinors (device).  s_dev (device, caller-owned,
+ * 12V x 12L^3 complex128 = 2304 T L^6 x 16 bytes): dagger = 0 -> double [T][L^3][12][L^3][12][2];
+ * dagger = 1 -> the Hermitian conjugate, double [L^3][12][T][L^3][12][2].  All sources in one pass (the array is written once).
+ * fp64.  Asynchronous on `stream`. */
+int stochastic_fill(const double *x_dev, const double *eta_dev, const int dims[4], int n_rhs, int t0, double scale, int dagger,
+                    double *s_dev, void *stream);
+
 /* ---- measurement helpers (internal layout, no reorders; used by bench.py and the ncu runs) ---- */
 enum {
     CLOVER_KERNEL_HOP = 0,        /* out_e = H_eo in_o                          (1320 flop/site)  */

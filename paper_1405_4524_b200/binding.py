@@ -18,7 +18,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 OP_HOP_EO, OP_HOP_OE, OP_HOP_FULL, OP_CLOVER, OP_CLOVER_INV, OP_D_FULL, OP_MHAT = range(7)
 KERNEL_HOP, KERNEL_AINV_HOP, KERNEL_A_MINUS_HOP = range(3)
 EXPORTS = ["clover_create", "clover_destroy", "dslash_apply", "clover_solve", "clover_solve_host", "noise_fill",
-           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator"]
+           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill"]
 
 
 class ClovOpts(ctypes.Structure):
@@ -50,6 +50,7 @@ _lib.clover_get_stats.argtypes = [_vp, ctypes.POINTER(SolveStats)]
 _lib.clover_last_error.argtypes = [_vp]
 _lib.stochastic_operators.argtypes = [_vp, _vp, _ip, _i, _vp, _vp]
 _lib.stochastic_correlator.argtypes = [_vp, _i, _i, _d, _vp, _vp]
+_lib.stochastic_fill.argtypes = [_vp, _vp, _ip, _i, _i, _d, _i, _vp, _vp]
 _lib.clover_last_error.restype = ctypes.c_char_p
 
 
@@ -113,6 +114,22 @@ def stochastic_correlator(o, scale=1.0):
     c = torch.empty((T, T), dtype=torch.complex128, device="cuda")
     _check(_lib.stochastic_correlator(o.data_ptr(), T, n, float(scale), c.data_ptr(), _stream()))
     return c
+
+
+def stochastic_fill(x, eta, t0=0, scale=1.0, dagger=False, out=None):
+    """S[t, z3, a, x3, b] = (1/(n scale^2)) sum_i X_i(t, z3, a) conj(eta_i(t0, x3, b)) (paper eq. 7.3); dagger=True returns the
+    Hermitian conjugate [x3, b, t, z3, a].  x, eta complex128 [n, T, Z, Y, X, 4, 3] on the device."""
+    _require_cuda()
+    assert x.is_cuda and eta.is_cuda and x.is_contiguous() and eta.is_contiguous() and x.dtype == eta.dtype == torch.complex128
+    assert x.shape == eta.shape
+    n, T, Z, Y, X = x.shape[:5]
+    V3 = Z * Y * X
+    shape = (V3, 12, T, V3, 12) if dagger else (T, V3, 12, V3, 12)
+    if out is None:
+        out = torch.empty(shape, dtype=torch.complex128, device="cuda")
+    assert tuple(out.shape) == shape and out.is_contiguous()
+    _check(_lib.stochastic_fill(x.data_ptr(), eta.data_ptr(), _i4((X, Y, Z, T)), n, int(t0), float(scale), int(dagger), out.data_ptr(), _stream()))
+    return out
 
 
 class Clover:

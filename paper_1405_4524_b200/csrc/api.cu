@@ -135,6 +135,18 @@ int stochastic_correlator(const double *o_dev, int T, int n_rhs, double scale, d
     return launch_correlator(o_dev, T, n_rhs, scale, c_dev, (cudaStream_t)stream);
 }
 
+int stochastic_fill(const double *x_dev, const double *eta_dev, const int dims[4], int n_rhs, int t0, double scale, int dagger, double *s_dev,
+                    void *stream)
+{
+    if (!x_dev || !eta_dev || !s_dev) { set_error("stochastic_fill: null argument"); return CLOVER_EINVAL; }
+    CLV_CHECK(check_dims(dims));
+    if (n_rhs < 1 || t0 < 0 || t0 >= dims[3] || !(scale > 0.0)) { set_error("stochastic_fill: bad n_rhs, t0 or scale"); return CLOVER_EINVAL; }
+    const long long rows = 12LL * dims[0] * dims[1] * dims[2] * dims[3];
+    if (rows / 64 + 1 > 65535) { set_error("stochastic_fill: lattice too large (the 12V x 12L^3 array would not fit any GPU)"); return CLOVER_EINVAL; }
+    CLV_CHECK(check_device());
+    return launch_fill(x_dev, eta_dev, dims, n_rhs, t0, scale, dagger != 0, s_dev, (cudaStream_t)stream);
+}
+
 int clover_bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms_per_launch, void *stream)
 {
     if (!ctx || !ms_per_launch) { set_error("clover_bench_kernel: null argument"); return CLOVER_EINVAL; }

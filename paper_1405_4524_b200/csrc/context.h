@@ -86,6 +86,9 @@ int launch_noise(void *out, int precision, const int dims[4], uint64_t seed, int
 int launch_contract(const double *eta, const double *xs, const int dims[4], int n, double *o, cudaStream_t st);
 int launch_correlator(const double *o, int T, int n, double scale, double *c, cudaStream_t st);
 
+// ---- fill.cu ----
+int launch_fill(const double *x, const double *eta, const int dims[4], int n, int t0, double scale, int dagger, double *s, cudaStream_t st);
+
 // ---- solver.cu ----
 int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, double tol, int max_iter, int batch, int mixed,
                   clover_rhs_info *info, cudaStream_t st, int host_buffers);
