@@ -21,7 +21,8 @@ struct SolveWork {
     int partial_blocks = 0;
     double *stage = nullptr;
     unsigned *ticket = nullptr;
-    RhsScalars *sc_dev = nullptr, *sc_host = nullptr;
+    RhsScalars *sc_dev = nullptr, *sc_host = nullptr;  // sc_host: mapped pinned memory the device writes the flags into
+    RhsScalars *sc_host_dev = nullptr;                 // device address of sc_host
     // host-buffer solves: double-buffered canonical staging, copies on their own streams so that the H2D of batch i+1 and the
     // D2H of batch i-1 overlap the solve of batch i
     double *stage_in[2] = {}, *stage_out[2] = {};
@@ -85,7 +86,8 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
         if (!W->sc_dev) {
             CLV_CUDA(cudaMalloc(&W->sc_dev, 8 * sizeof(RhsScalars)));
             CLV_CUDA(cudaMemset(W->sc_dev, 0, 8 * sizeof(RhsScalars)));
-            CLV_CUDA(cudaMallocHost(&W->sc_host, 8 * sizeof(RhsScalars)));
+            CLV_CUDA(cudaHostAlloc((void **)&W->sc_host, 8 * sizeof(RhsScalars), cudaHostAllocMapped));
+            CLV_CUDA(cudaHostGetDevicePointer((void **)&W->sc_host_dev, W->sc_host, 0));
             CLV_CUDA(cudaMalloc(&W->stage, 8 * 32 * 4 * sizeof(double)));
             CLV_CUDA(cudaMalloc(&W->ticket, 8 * sizeof(unsigned)));
             CLV_CUDA(cudaMemset(W->ticket, 0, 8 * sizeof(unsigned)));
@@ -176,9 +178,25 @@ static int mhat(clover_ctx *ctx, int B, const typename Vec<R>::T *in, typename V
     return 0;
 }
 
+// Flag read-back: a 32-thread kernel stores the per-rhs scalars straight into mapped pinned host memory.  (A cudaMemcpyAsync
+// would queue behind the gigabyte device-to-host copies of clover_solve_host on the copy engine and stall every iteration.)
+__global__ void publish_scalars_kernel(const RhsScalars *__restrict__ src, RhsScalars *dst, int words)
+{
+    const unsigned long long *s = reinterpret_cast<const unsigned long long *>(src);
+    volatile unsigned long long *d = reinterpret_cast<volatile unsigned long long *>(dst);
+    for (int i = threadIdx.x; i < words; i += blockDim.x) d[i] = s[i];
+    __threadfence_system();
+}
+static int publish_scalars(SolveWork *W, int B, cudaStream_t st)
+{
+    static_assert(sizeof(RhsScalars) % 8 == 0, "RhsScalars is copied in 8-byte words");
+    publish_scalars_kernel<<<1, 32, 0, st>>>(W->sc_dev, W->sc_host_dev, B * (int)(sizeof(RhsScalars) / 8));
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
 static int fetch_scalars(SolveWork *W, int B, cudaStream_t st)
 {
-    CLV_CUDA(cudaMemcpyAsync(W->sc_host, W->sc_dev, B * sizeof(RhsScalars), cudaMemcpyDeviceToHost, st));
+    CLV_CHECK(publish_scalars(W, B, st));
     CLV_CUDA(cudaStreamSynchronize(st));
     return 0;
 }
@@ -269,7 +287,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         CLV_CHECK(blas_scalar_step(bc, SC_OMEGA, grid, tol2, delta2));
         CLV_CHECK(blas_xr_update<R>(bc, x, r, p, s, t, r0, &nb));
         CLV_CHECK(blas_scalar_step(bc, SC_RHO, nb, tol2, delta2));
-        CLV_CUDA(cudaMemcpyAsync(W->sc_host, W->sc_dev, B * sizeof(RhsScalars), cudaMemcpyDeviceToHost, st));
+        CLV_CHECK(publish_scalars(W, B, st));
         return 0;
     };
     if (use_graph && (!W->iter_graph || W->graph_B != B || W->graph_prec != (int)sizeof(R) || W->graph_tol2 != tol2 || W->graph_delta2 != delta2)) {
