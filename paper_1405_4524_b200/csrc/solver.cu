@@ -205,7 +205,7 @@ static double reliable_delta()
 {
     const char *e = getenv("CLOVER_DELTA");  // tuning/debug knob only
     const double d = e ? atof(e) : 0.0;
-    return (d > 0.0 && d < 1.0) ? d : 1e-3;
+    return (d > 0.0 && d < 1.0) ? d : 1e-4;
 }
 
 // Small lattices are launch-bound (a 16^3x32 Dslash takes ~10 us): replay the iteration as a CUDA graph there.
