@@ -1,13 +1,66 @@
 // dslash_inst.cuh -- host dispatch of one (precision, batch) family of Dslash kernels; included by the
 // dslash_<prec>_b<B>.cu instantiation units so the variants compile in parallel.
 #pragma once
-#include "dslash_kernel.cuh"
+#include "dslash2_kernel.cuh"
+#include <cstdlib>
 
 namespace clv {
+
+// fp32, B >= 2: the (site, rhs-pair) kernel of dslash2_kernel.cuh
+template <int B, int RECON>
+static int launch_dslash2_BR(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
+{
+    const Geom &g = ctx->geom;
+    const unsigned npairs = (unsigned)g.Vh * B / 2;
+    const unsigned grid = (npairs + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
+    if (grid_out) *grid_out = (int)grid;
+    const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
+#define CLV_LAUNCH2(XM, PI, DT)                                                      \
+    case (XM) * 100 + (PI) * 10 + (DT):                                              \
+        dslash2_kernel<B, RECON, XM, PI, DT><<<grid, DSLASH_BLOCK, 0, st>>>(g, op, a); \
+        break;
+    switch (key) {
+        CLV_LAUNCH2(XM_NONE, 0, DOT_NONE)
+        CLV_LAUNCH2(XM_NONE, 1, DOT_NONE)
+        CLV_LAUNCH2(XM_PLAIN, 0, DOT_NONE)
+        CLV_LAUNCH2(XM_PLAIN, 1, DOT_NONE)
+        CLV_LAUNCH2(XM_CLOVER, 0, DOT_NONE)
+        CLV_LAUNCH2(XM_CLOVER, 0, DOT_W)
+        CLV_LAUNCH2(XM_CLOVER, 0, DOT_X)
+        CLV_LAUNCH2(XM_CLOVER, 0, DOT_RES)
+    default:
+        set_error("dslash: unsupported variant xmode=%d pinv=%d dot=%d", a.xmode, a.pinv, a.dot);
+        return CLOVER_EINVAL;
+    }
+#undef CLV_LAUNCH2
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R, int B, int RECON> struct PairLaunch {   // double, or B = 1: no pair kernel
+    static bool use() { return false; }
+    static int go(const clover_ctx *, const OpData<R> &, const DslashArgs<R> &, cudaStream_t, int *) { return CLOVER_EINVAL; }
+};
+template <int B, int RECON> struct PairLaunchF {
+    static bool use()
+    {
+        static const bool on = [] { const char *e = getenv("CLOVER_R2"); return e ? atoi(e) != 0 : true; }();  // tuning/debug knob only
+        return on;
+    }
+    static int go(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
+    {
+        return launch_dslash2_BR<B, RECON>(ctx, op, a, st, grid_out);
+    }
+};
+template <int RECON> struct PairLaunch<float, 2, RECON> : PairLaunchF<2, RECON> {};
+template <int RECON> struct PairLaunch<float, 4, RECON> : PairLaunchF<4, RECON> {};
+template <int RECON> struct PairLaunch<float, 8, RECON> : PairLaunchF<8, RECON> {};
+
 
 template <typename R, int B, int RECON>
 static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const DslashArgs<R> &a, cudaStream_t st, int *grid_out)
 {
+    // the pair kernel wins where link AND clover loads are shared (the fused solver kernels); the plain hop stays per-rhs
+    if (PairLaunch<R, B, RECON>::use() && (a.xmode != XM_NONE || a.pinv)) return PairLaunch<R, B, RECON>::go(ctx, op, a, st, grid_out);
     const Geom &g = ctx->geom;
     const unsigned n = (unsigned)g.Vh * B;
     const unsigned grid = (n + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
