@@ -8,14 +8,15 @@
 // layout, moves with one 256-bit load or store (LDG.E.ENL2.256 on sm_100), so the spinor wavefronts per rhs do not grow.
 #pragma once
 #include "dslash_kernel.cuh"
+#include <cuda_pipeline.h>
 
 namespace clv {
 
 #ifndef CLV_R2_MINB
 #define CLV_R2_MINB 3
 #endif
-#ifndef CLV_R2_PIPE
-#define CLV_R2_PIPE 0
+#ifndef CLV_R2_SMEM
+#define CLV_R2_SMEM 1   // stage the CTA's clover blocks in shared memory with cp.async at kernel start
 #endif
 
 __device__ __forceinline__ void ldg256(const float4 *p, float4 &a, float4 &b)
@@ -89,16 +90,23 @@ template <int RECON, int MU, int FWD> __device__ __forceinline__ void hop_comput
     accB.template add<MU, FWD>(hB, d.u);
 }
 
-// yA (+)= M xA, yB (+)= M xB with one load of the packed blocks
+// yA (+)= M xA, yB (+)= M xB with one load of the packed blocks; `srow` != nullptr: the site's 18 float4 rows staged in shared memory
 template <bool ACCUM>
-__device__ __forceinline__ void clover_mul2(const float2 *__restrict__ clov, unsigned cb, const cx<float> xA[12], cx<float> yA[12],
+__device__ __forceinline__ void clover_mul2(const float2 *__restrict__ clov, unsigned cb, const float4 *srow, const cx<float> xA[12], cx<float> yA[12],
                                             const cx<float> xB[12], cx<float> yB[12])
 {
 #pragma unroll
     for (int blk = 0; blk < 2; blk++) {
         const int o = 6 * blk;
         cx<float> m[18];
-        load_clover_block(clov, cb, blk, m);
+        if (CLV_R2_SMEM) {
+#pragma unroll
+            for (int k = 0; k < 9; k++) {
+                const float4 v = srow[9 * blk + k];
+                m[2 * k] = mk<float>(v.x, v.y);
+                m[2 * k + 1] = mk<float>(v.z, v.w);
+            }
+        } else load_clover_block(clov, cb, blk, m);
 #pragma unroll
         for (int k = 0; k < 3; k++) {
             if (ACCUM) {
@@ -183,38 +191,44 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, CLV_R2_MINB) dslash2_kernel(cons
     const unsigned j = 2u * (blockIdx.x * DSLASH_BLOCK + threadIdx.x);   // first rhs of this thread's pair
     const bool active = j < (unsigned)g.Vh * B;
     double dA[3] = {0, 0, 0}, dB[3] = {0, 0, 0};
+    const int p = a.parity;
+    constexpr int SITES = 2 * DSLASH_BLOCK / B;   // sites of this CTA: consecutive cb from blockIdx.x * SITES
+    __shared__ __align__(16) float4 cl_s[(CLV_R2_SMEM && (XMODE == XM_CLOVER || PINV)) ? SITES * 18 : 1];
+    if (CLV_R2_SMEM && (XMODE == XM_CLOVER || PINV)) {
+        // the one clover field this variant needs (A for X = A x, A^-1 for P): 288 bytes per site, 16-byte async copies whose
+        // DRAM latency is hidden behind the whole hop; consecutive threads copy consecutive sites of one row (coalesced)
+        const float2 *clov = PINV ? (p ? op.clov_inv[1] : op.clov_inv[0]) : (p ? op.clov[1] : op.clov[0]);
+        const float4 *base4 = reinterpret_cast<const float4 *>(clov);
+        const unsigned cb0 = blockIdx.x * SITES;
+        for (int item = threadIdx.x; item < SITES * 18; item += DSLASH_BLOCK) {
+            const int row = item / SITES, site = item % SITES;
+            const unsigned cbs = cb0 + site;
+            if (cbs < (unsigned)g.Vh) __pipeline_memcpy_async(&cl_s[site * 18 + row], base4 + ((size_t)(cbs >> 5) * 18 + row) * 32 + (cbs & 31u), 16);
+        }
+        __pipeline_commit();
+    }
+    HopAcc<float> hA, hB;
+    int cb = 0;
     if (active) {
-        const int cb = j / B, rhs = j % B, p = a.parity;
+        cb = j / B;
+        const int rhs = j % B;
         const Coord c = decode(g, cb, p);
-        HopAcc<float> hA, hB;
         hA.zero();
         hB.zero();
-        prefetch_epilogue<float, XMODE, PINV, DOT>(op, a, p, cb, j);   // the pair shares its 128-byte lines
-        if constexpr (CLV_R2_PIPE) {   // loads of direction d+1 issued before the arithmetic of direction d
-            HopIn2 e0, e1;
-            hop_load2<B, RECON, 0, 1>(g, op, a.in, p, cb, rhs, c, e0);
-            hop_load2<B, RECON, 0, 0>(g, op, a.in, p, cb, rhs, c, e1);
-            hop_compute2<RECON, 0, 1>(e0, hA, hB);
-            hop_load2<B, RECON, 1, 1>(g, op, a.in, p, cb, rhs, c, e0);
-            hop_compute2<RECON, 0, 0>(e1, hA, hB);
-            hop_load2<B, RECON, 1, 0>(g, op, a.in, p, cb, rhs, c, e1);
-            hop_compute2<RECON, 1, 1>(e0, hA, hB);
-            hop_load2<B, RECON, 2, 1>(g, op, a.in, p, cb, rhs, c, e0);
-            hop_compute2<RECON, 1, 0>(e1, hA, hB);
-            hop_load2<B, RECON, 2, 0>(g, op, a.in, p, cb, rhs, c, e1);
-            hop_compute2<RECON, 2, 1>(e0, hA, hB);
-            hop_load2<B, RECON, 3, 1>(g, op, a.in, p, cb, rhs, c, e0);
-            hop_compute2<RECON, 2, 0>(e1, hA, hB);
-            hop_load2<B, RECON, 3, 0>(g, op, a.in, p, cb, rhs, c, e1);
-            hop_compute2<RECON, 3, 1>(e0, hA, hB);
-            hop_compute2<RECON, 3, 0>(e1, hA, hB);
-        } else
+        prefetch_epilogue<float, (CLV_R2_SMEM && XMODE == XM_CLOVER ? XM_PLAIN : XMODE), (CLV_R2_SMEM ? 0 : PINV), DOT>(op, a, p, cb, j);   // x and w lines (the pair shares them)
         {
             HopIn2 d;
 #define CLV_HOP2(MU, FW) hop_load2<B, RECON, MU, FW>(g, op, a.in, p, cb, rhs, c, d); hop_compute2<RECON, MU, FW>(d, hA, hB);
             CLV_HOP2(0, 1) CLV_HOP2(0, 0) CLV_HOP2(1, 1) CLV_HOP2(1, 0) CLV_HOP2(2, 1) CLV_HOP2(2, 0) CLV_HOP2(3, 1) CLV_HOP2(3, 0)
 #undef CLV_HOP2
         }
+    }
+    if (CLV_R2_SMEM && (XMODE == XM_CLOVER || PINV)) {
+        __pipeline_wait_prior(0);
+        __syncthreads();
+    }
+    if (active) {
+        const float4 *srow = cl_s + (cb - blockIdx.x * SITES) * 18;
         cx<float> accA[12], accB[12];
         hA.finish(accA);
         hB.finish(accB);
@@ -232,10 +246,10 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, CLV_R2_MINB) dslash2_kernel(cons
                 accB[i] = accB[i] + xB[i];
             }
         }
-        if (XMODE == XM_CLOVER) clover_mul2<true>(p ? op.clov[1] : op.clov[0], cb, xA, accA, xB, accB);
+        if (XMODE == XM_CLOVER) clover_mul2<true>(p ? op.clov[1] : op.clov[0], cb, srow, xA, accA, xB, accB);
         if (PINV) {
             cx<float> tA[12], tB[12];
-            clover_mul2<false>(p ? op.clov_inv[1] : op.clov_inv[0], cb, accA, tA, accB, tB);
+            clover_mul2<false>(p ? op.clov_inv[1] : op.clov_inv[0], cb, srow, accA, tA, accB, tB);
 #pragma unroll
             for (int i = 0; i < 12; i++) {
                 accA[i] = tA[i];
