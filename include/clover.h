@@ -52,7 +52,7 @@ typedef struct {
 } clover_opts;
 
 typedef struct {
-    int status;           /* 0 converged, 1 max_iter reached, 2 breakdown, 3 non-finite */
+    int status;           /* 0 converged, 1 max_iter reached, 2 repeated breakdown (<r0,v> = 0 after 8 restarts), 3 non-finite */
     int iters;            /* BiCGStab iterations of the batch this source was in */
     int reliable_updates; /* fp64 residual recomputations of that batch */
     double iter_resid;    /* last fp64 even-odd residual ||b_e - Mhat y|| / ||eta|| */

@@ -102,6 +102,14 @@ __global__ void __launch_bounds__(BLAS_BLOCK) xr_update_kernel(size_t n, int B, 
     block_reduce(B, d0, d1, d2, partial);
 }
 
+// ---- r0 = r for the rhs flagged `restart` ------------------------------------------------------------
+template <typename V> __global__ void __launch_bounds__(BLAS_BLOCK) restart_kernel(size_t n, int B, const RhsScalars *__restrict__ sc, const V *__restrict__ r,
+                                                                                    V *__restrict__ r0)
+{
+    if (!sc[threadIdx.x & (B - 1)].restart) return;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) r0[i] = r[i];
+}
+
 // ---- p = r + beta (p - omega v) ---------------------------------------------------------------------
 template <typename V> __global__ void __launch_bounds__(BLAS_BLOCK) p_update_kernel(size_t n, int B, const RhsScalars *__restrict__ sc, V *__restrict__ p,
                                                                                      const V *__restrict__ r, const V *__restrict__ v)
@@ -264,6 +272,8 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         q.alpha = q.omega = q.beta = make_double2(0., 0.);
         q.want_update = 0;
         q.claim = 0;
+        q.restart = 0;
+        q.nrestart = 0;
         if (!(q.eta2 > 0.) || d0 <= tol2 * q.eta2) q.done = 1;  // zero source or already converged
         if (!isfinite(d0)) { q.done = 1; q.status = 3; }
         break;
@@ -272,8 +282,15 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         if (!q.done) {
             const zs r0v{d0, d1};
             if (!finite_z(r0v)) { q.done = 1; q.status = 3; }
-            else if (!(d0 * d0 + d1 * d1 > 0.)) { q.done = 1; q.status = 2; }
-            else al = zdiv(ld_z(q.rho), r0v);
+            else if (!(d0 * d0 + d1 * d1 > 0.)) {
+                // breakdown (e.g. a point source on unit links): this iteration becomes a pure minimal-residual step (alpha = 0),
+                // then the recurrence restarts from the current residual, r0 := r (same remedy as the oracle, R11)
+                if (q.nrestart < 8) { q.restart = 1; q.nrestart++; }
+                else { q.done = 1; q.status = 2; }
+            } else {
+                al = zdiv(ld_z(q.rho), r0v);
+                if (!finite_z(al)) { al = zero; if (q.nrestart < 8) { q.restart = 1; q.nrestart++; } else { q.done = 1; q.status = 2; } }
+            }
         }
         q.alpha = st_z(al);
         break;
@@ -319,6 +336,9 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             else if (d0 <= tol2 * q.eta2) { q.done = 1; q.beta = st_z(zero); }
         }
         break;
+    case SC_RESTART:  // after r0 := r: rho = <r0, r> = ||r||^2 (the value SC_RHO / SC_TRUE left in r2)
+        if (q.restart) { q.rho = make_double2(q.r2, 0.); q.beta = st_z(zero); q.restart = 0; }
+        break;
     case SC_FINAL:  // d0 + d1 = ||eta - D psi||^2 on the full lattice; stored in r2 (true_r2 keeps the even-odd value)
         q.r2 = d0 + d1;
         break;
@@ -352,6 +372,14 @@ template <typename R> int blas_p_update(const BlasCtx &c, typename Vec<R>::T *p,
 {
     const size_t n = field_vecs<R>(*c.g, c.B);
     p_update_kernel<<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, p, r, v);
+    BLAS_LAUNCHED(c);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R> int blas_restart(const BlasCtx &c, const typename Vec<R>::T *r, typename Vec<R>::T *r0)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    restart_kernel<<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, r, r0);
     BLAS_LAUNCHED(c);
     CLV_CUDA(cudaGetLastError());
     return 0;
@@ -397,6 +425,7 @@ int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, doubl
     template int blas_xr_update<R>(const BlasCtx &, Vec<R>::T *, Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *,          \
                                    const Vec<R>::T *, int *);                                                                                    \
     template int blas_p_update<R>(const BlasCtx &, Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *);                                           \
+    template int blas_restart<R>(const BlasCtx &, const Vec<R>::T *, Vec<R>::T *);                                                                \
     template int blas_accumulate_y<R>(const BlasCtx &, double2 *, Vec<R>::T *);                                                                  \
     template int blas_residual<R>(const BlasCtx &, const double2 *, const double2 *, double2 *, Vec<R>::T *, int *);
 INST(float)

@@ -35,7 +35,9 @@ template <typename R> int blas_residual(const BlasCtx &c, const double2 *b, cons
 int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, const double2 *a2, const double2 *b2, int *nblocks);
 
 // scalar steps (one block per rhs): reduce the partials of `nblocks` blocks and update RhsScalars
-enum { SC_ETA2 = 0, SC_INIT = 1, SC_ALPHA = 2, SC_OMEGA = 3, SC_RHO = 4, SC_TRUE = 5, SC_FINAL = 6 };
+enum { SC_ETA2 = 0, SC_INIT = 1, SC_ALPHA = 2, SC_OMEGA = 3, SC_RHO = 4, SC_TRUE = 5, SC_FINAL = 6, SC_RESTART = 7 };
+// r0 = r for the rhs whose `restart` flag is set (breakdown recovery)
+template <typename R> int blas_restart(const BlasCtx &c, const typename Vec<R>::T *r, typename Vec<R>::T *r0);
 int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2);
 
 }  // namespace clv

@@ -26,6 +26,8 @@ struct RhsScalars {
     int want_update;  // 1 if this rhs asks for a reliable update (||r|| < delta max||r||, or stagnation)
     int status;       // clover_rhs_info.status
     int claim;        // 1 if the iterated residual of this rhs meets the tolerance (to be confirmed in fp64)
+    int restart;      // 1 if <r0, v> vanished this iteration: r0 := r, rho := ||r||^2 before the next one (R11)
+    int nrestart;     // restarts so far (a rhs that keeps breaking down ends with status 2)
 };
 
 struct SolveWork;  // solver.cu

@@ -341,6 +341,14 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             updates++;
             claim_age = 0;
         }
+        {   // breakdown recovery (R11): r0 := r, rho := ||r||^2 for the rhs that asked for it; beta is already 0 so p := r next
+            bool any_restart = false;
+            for (int i = 0; i < B; i++) any_restart |= !W->sc_host[i].done && W->sc_host[i].restart;
+            if (any_restart) {
+                CLV_CHECK(blas_restart<R>(bc, r, r0));
+                CLV_CHECK(blas_scalar_step(bc, SC_RESTART, 0, tol2, delta2));
+            }
+        }
     }
     CLV_CUDA(cudaEventRecord(W->ev[3], st));
     // odd sites and verification on the full lattice, all fp64
