@@ -235,7 +235,8 @@ def main():
     tp = os.path.join(ROOT, "profiles", "traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
         traffic = json.load(open(tp)).get(f"a_minus_hop_{cfg['name']}_b{batch}")
-    roofline = {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if cfg['mixed'] else 'double'},B={batch},recon={g},A x - k^2 H t,+dots>",
+    roofline = {"bound": "hbm", "kernel": (f"dslash2_kernel<B={batch},recon={g},A x - k^2 H t,+dots> (fp32, one thread per site and rhs pair)" if cfg["mixed"] and batch >= 2
+                           else f"dslash_kernel<{'float' if cfg['mixed'] else 'double'},B={batch},recon={g},A x - k^2 H t,+dots>"),
                 "achieved": ach, "timed": timed, "peak": peaks["hbm_gbs"], "peak_kind": peak_kind, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                 "traffic": traffic, "algorithmic_bytes_per_site_rhs": bytes_a_minus, "us_per_launch": t_a_minus * 1e6,
                 "gflops": 1872.0 * Vh * batch / t_a_minus / 1e9,
