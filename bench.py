@@ -312,6 +312,14 @@ def main():
             c1.record()
             torch.cuda.synchronize()
             times[dag] = c0.elapsed_time(c1) / 3 * 1e-3
+        B.timeslice_norm2(fs, 1, 16)
+        torch.cuda.synchronize()
+        c0.record()
+        for _ in range(3):
+            B.timeslice_norm2(fs, 1, 16)
+        c1.record()
+        torch.cuda.synchronize()
+        t_trace = c0.elapsed_time(c1) / 3 * 1e-3
         fbytes = fs.numel() * 16
         fflop = 8.0 * fs.numel() * n_rhs
         fp64_peak = 148 * 64 * 2 * 1.965e9
@@ -319,6 +327,9 @@ def main():
                     "ms_fill": times[0] * 1e3, "ms_fill_dagger": times[1] * 1e3, "write_gbs": fbytes / times[0] / 1e9,
                     "tflops_fp64": fflop / times[0] / 1e12, "frac_fp64_alu": fflop / times[0] / fp64_peak,
                     "frac_hbm_write": fbytes / times[0] / 1e9 / peaks["hbm_gbs"], "ms_per_source_both": (times[0] + times[1]) * 1e3 / n_rhs,
+                    "trace": {"what": "sum_x sum_z Tr S_s S_s^+ for all 16 timeslices (Table I last row)", "ms": t_trace * 1e3,
+                              "read_gbs": fbytes / t_trace / 1e9, "frac_hbm": fbytes / t_trace / 1e9 / peaks["hbm_gbs"],
+                              "paper_table1_s_per_timeslice": 43.3},
                     "paper_table2_s_per_source": {"cpu": 100.8, "gpu": 8.8, "hardware": "unnamed", "cite": "PAPER.md L340-344"}}
         del fs, fe, fx
 

@@ -123,6 +123,13 @@ int stochastic_correlator(const double *o_dev, int T, int n_rhs, double scale, d
 int stochastic_fill(const double *x_dev, const double *eta_dev, const int dims[4], int n_rhs, int t0, double scale, int dagger,
                     double *s_dev, void *stream);
 
+/* ---- trace operations of Table I (S 8(f) rank 3) ---- */
+/* out[t] = sum_{o < n_outer} sum_{k < slice_len} |f[o][t][k]|^2 for a complex128 device field viewed as [n_outer][T][slice_len]:
+ * with f = 12 point-source solutions (n_outer = 12, slice_len = 12 L^3) this is sum_y Tr[S_p(t,y;0,0) S_p^+(t,y;0,0)], the
+ * zero-momentum pion correlator; with f = the array of stochastic_fill (n_outer = 1, slice_len = 144 L^6) it is
+ * sum_x sum_z Tr[S_s(t,z;0,x) S_s^+(t,z;0,x)].  out_dev: double [T] (device).  fp64, deterministic.  Asynchronous on `stream`. */
+int timeslice_norm2(const double *f_dev, long long n_outer, int T, long long slice_len, double *out_dev, void *stream);
+
 /* ---- measurement helpers (internal layout, no reorders; used by bench.py and the ncu runs) ---- */
 enum {
     CLOVER_KERNEL_HOP = 0,        /* out_e = H_eo in_o                          (1320 flop/site)  */

@@ -18,7 +18,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 OP_HOP_EO, OP_HOP_OE, OP_HOP_FULL, OP_CLOVER, OP_CLOVER_INV, OP_D_FULL, OP_MHAT = range(7)
 KERNEL_HOP, KERNEL_AINV_HOP, KERNEL_A_MINUS_HOP = range(3)
 EXPORTS = ["clover_create", "clover_destroy", "dslash_apply", "clover_solve", "clover_solve_host", "noise_fill",
-           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill"]
+           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill", "timeslice_norm2"]
 
 
 class ClovOpts(ctypes.Structure):
@@ -51,6 +51,7 @@ _lib.clover_last_error.argtypes = [_vp]
 _lib.stochastic_operators.argtypes = [_vp, _vp, _ip, _i, _vp, _vp]
 _lib.stochastic_correlator.argtypes = [_vp, _i, _i, _d, _vp, _vp]
 _lib.stochastic_fill.argtypes = [_vp, _vp, _ip, _i, _i, _d, _i, _vp, _vp]
+_lib.timeslice_norm2.argtypes = [_vp, ctypes.c_longlong, _i, ctypes.c_longlong, _vp, _vp]
 _lib.clover_last_error.restype = ctypes.c_char_p
 
 
@@ -129,6 +130,15 @@ def stochastic_fill(x, eta, t0=0, scale=1.0, dagger=False, out=None):
         out = torch.empty(shape, dtype=torch.complex128, device="cuda")
     assert tuple(out.shape) == shape and out.is_contiguous()
     _check(_lib.stochastic_fill(x.data_ptr(), eta.data_ptr(), _i4((X, Y, Z, T)), n, int(t0), float(scale), int(dagger), out.data_ptr(), _stream()))
+    return out
+
+
+def timeslice_norm2(f, n_outer, T):
+    """out[t] = sum |f[o, t, :]|^2 for a complex128 device tensor viewed as [n_outer, T, -1] (Table I traces)."""
+    _require_cuda()
+    assert f.is_cuda and f.is_contiguous() and f.dtype == torch.complex128 and f.numel() % (n_outer * T) == 0
+    out = torch.empty(T, dtype=torch.float64, device="cuda")
+    _check(_lib.timeslice_norm2(f.data_ptr(), n_outer, T, f.numel() // (n_outer * T), out.data_ptr(), _stream()))
     return out
 
 

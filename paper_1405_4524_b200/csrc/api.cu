@@ -147,6 +147,14 @@ int stochastic_fill(const double *x_dev, const double *eta_dev, const int dims[4
     return launch_fill(x_dev, eta_dev, dims, n_rhs, t0, scale, dagger != 0, s_dev, (cudaStream_t)stream);
 }
 
+int timeslice_norm2(const double *f_dev, long long n_outer, int T, long long slice_len, double *out_dev, void *stream)
+{
+    if (!f_dev || !out_dev) { set_error("timeslice_norm2: null argument"); return CLOVER_EINVAL; }
+    if (n_outer < 1 || T < 1 || T > 65535 || slice_len < 1) { set_error("timeslice_norm2: bad n_outer, T or slice_len"); return CLOVER_EINVAL; }
+    CLV_CHECK(check_device());
+    return launch_timeslice_norm2(f_dev, (long)n_outer, T, (long)slice_len, out_dev, (cudaStream_t)stream);
+}
+
 int clover_bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms_per_launch, void *stream)
 {
     if (!ctx || !ms_per_launch) { set_error("clover_bench_kernel: null argument"); return CLOVER_EINVAL; }

@@ -91,6 +91,9 @@ int launch_correlator(const double *o, int T, int n, double scale, double *c, cu
 // ---- fill.cu ----
 int launch_fill(const double *x, const double *eta, const int dims[4], int n, int t0, double scale, int dagger, double *s, cudaStream_t st);
 
+// ---- traces.cu ----
+int launch_timeslice_norm2(const double *f, long n_outer, int T, long slice_len, double *out, cudaStream_t st);
+
 // ---- solver.cu ----
 int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, double tol, int max_iter, int batch, int mixed,
                   clover_rhs_info *info, cudaStream_t st, int host_buffers);

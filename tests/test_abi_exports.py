@@ -17,7 +17,7 @@ def test_library_exports_every_declared_symbol():
     lib = ctypes.CDLL(build.build())
     names = _declared()
     assert {"clover_create", "clover_destroy", "dslash_apply", "clover_solve", "clover_solve_host", "noise_fill",
-            "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill"} <= set(names)
+            "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill", "timeslice_norm2"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n
 
