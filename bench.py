@@ -274,6 +274,20 @@ def main():
                "wall_s_per_step": (time.perf_counter() - t0) / args.steps}
         del h_eta, h_psi
 
+    # ---- H1 noise fill alone (a pure write stream: 192 B per site and source in fp64) ----
+    noise = None
+    if rank == 0:
+        B.noise_fill(dims, cfg["noise_seed"], n_rhs, rhs_offset=offset, time_dilution=cfg["dilution"], scale=wl.INV_SQRT2, out=eta)
+        torch.cuda.synchronize()
+        n0, n1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n0.record()
+        for _ in range(5):
+            B.noise_fill(dims, cfg["noise_seed"], n_rhs, rhs_offset=offset, time_dilution=cfg["dilution"], scale=wl.INV_SQRT2, out=eta)
+        n1.record()
+        torch.cuda.synchronize()
+        tn = n0.elapsed_time(n1) / 5 * 1e-3
+        noise = {"ms": tn * 1e3, "write_gbs": n_rhs * V * 192 / tn / 1e9, "frac_hbm": n_rhs * V * 192 / tn / 1e9 / peaks["hbm_gbs"]}
+
     # ---- NEXT row (S 8(f) rank 1): stochastic-operator contraction O_ij(t) of the step's sources and solutions ----
     contraction = None
     if rank == 0:
@@ -342,7 +356,7 @@ def main():
                       "eps": cfg["eps"], "recon": cfg["recon"], "time_dilution": cfg["dilution"],
                       "solver": "even-odd BiCGStab, fp32 iteration + fp64 reliable updates" if cfg["mixed"] else "even-odd BiCGStab fp64",
                       "l2": "fields per sweep (>= 255 MB at batch 8) exceed the 126 MB L2; the stand-alone hop timing flushes L2 between launches"},
-           "clocks": sampler.summary(), "gpu_launches": launches, "roofline": roofline, "dslash": dslash, "e2e": e2e, "next_contraction": contraction, "next_fill": fill_res,
+           "clocks": sampler.summary(), "gpu_launches": launches, "roofline": roofline, "dslash": dslash, "e2e": e2e, "noise_fill": noise, "next_contraction": contraction, "next_fill": fill_res,
            "solve": {"iters": [i["iters"] for i in last["infos"]][::batch], "reliable_updates": [i["reliable_updates"] for i in last["infos"]][::batch],
                      "max_true_resid": max(i["true_resid"] for i in last["infos"]),
                      "phase_ms_per_step": {k: v / args.steps for k, v in phases.items()}}}

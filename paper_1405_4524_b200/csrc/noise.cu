@@ -30,6 +30,7 @@ __global__ void __launch_bounds__(256) noise_kernel(R *__restrict__ out, uint64_
                                                     int rhs_offset, int dilution, R scale)
 {
     const uint64_t pairs_per_rhs = n12V / 2;
+    const bool aligned32 = (reinterpret_cast<uintptr_t>(out) & 31u) == 0;
     const uint64_t total = pairs_per_rhs * (uint64_t)n_rhs;
     for (uint64_t i = (uint64_t)blockIdx.x * 256 + threadIdx.x; i < total; i += (uint64_t)gridDim.x * 256) {
         const uint64_t j = i / pairs_per_rhs, n = 2 * (i % pairs_per_rhs);
@@ -45,6 +46,9 @@ __global__ void __launch_bounds__(256) noise_kernel(R *__restrict__ out, uint64_
         R *dst = out + (j * n12V + n) * 2;
         if (sizeof(R) == 4) {
             *reinterpret_cast<float4 *>(dst) = make_float4((float)v[0], (float)v[1], (float)v[2], (float)v[3]);
+        } else if (aligned32) {  // one 32-byte store per thread: a warp writes 1 KB contiguous
+            asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(dst), "d"((double)v[0]), "d"((double)v[1]), "d"((double)v[2]), "d"((double)v[3])
+                         : "memory");
         } else {
             *reinterpret_cast<double2 *>(dst) = make_double2((double)v[0], (double)v[1]);
             *reinterpret_cast<double2 *>(dst + 2) = make_double2((double)v[2], (double)v[3]);

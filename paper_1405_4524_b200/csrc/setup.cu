@@ -243,54 +243,72 @@ template <typename CT> struct CanonC;
 template <> struct CanonC<double> { typedef double2 T; };
 template <> struct CanonC<float> { typedef float2 T; };
 
-// thread = (parity, j = cb*B + rhs)
-template <typename CT, typename R> __global__ void reorder_in_kernel(Geom g, const CT *__restrict__ canon, typename Vec<R>::T *even,
-                                                                     typename Vec<R>::T *odd, int B)
+// One CTA of 384 threads moves one 32-lane block of j = cb*B + rhs (x 12 complex) through shared memory, so that both sides
+// are coalesced: the canonical side in 192-byte chunks (one (site, rhs) spinor each), the internal side in 512-byte rows.
+constexpr int RO_THREADS = 384;
+
+template <typename CT, typename R> __global__ void __launch_bounds__(RO_THREADS) reorder_in_kernel(Geom g, const CT *__restrict__ canon, typename Vec<R>::T *even,
+                                                                                                  typename Vec<R>::T *odd, int B)
 {
-    const unsigned j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= (unsigned)g.Vh * B) return;
-    const int p = blockIdx.y, cb = j / B, rhs = j % B;
+    __shared__ double2 sm[12][33];
+    const int p = blockIdx.y;
     const long V = 2L * g.Vh;
-    const typename CanonC<CT>::T *src = reinterpret_cast<const typename CanonC<CT>::T *>(canon) + ((long)rhs * V + lex_index(g, lex_of(g, cb, p))) * 12;
-    cx<R> psi[12];
-#pragma unroll
-    for (int k = 0; k < 12; k++) {
-        typename CanonC<CT>::T v = __ldg(src + k);
-        psi[k] = mk<R>((R)v.x, (R)v.y);
+    {
+        const int chunk = threadIdx.x / 12, k = threadIdx.x % 12;
+        const unsigned j = blockIdx.x * 32u + chunk;
+        double2 v = make_double2(0., 0.);
+        if (j < (unsigned)g.Vh * B) {
+            const int cb = j / B, rhs = j % B;
+            const typename CanonC<CT>::T e = __ldg(reinterpret_cast<const typename CanonC<CT>::T *>(canon) + ((long)rhs * V + lex_index(g, lex_of(g, cb, p))) * 12 + k);
+            v = make_double2((double)e.x, (double)e.y);
+        }
+        sm[k][chunk] = v;
     }
-    store_spinor(p ? odd : even, j, psi);
+    __syncthreads();
+    typename Vec<R>::T *f = p ? odd : even;
+    const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;   // 12 rows of 32 lanes
+    if (sizeof(R) == 8) {
+        reinterpret_cast<double2 *>(f)[((size_t)blockIdx.x * 12 + row) * 32 + lane] = sm[row][lane];
+    } else if (row < 6) {
+        const double2 a = sm[2 * row][lane], b = sm[2 * row + 1][lane];
+        reinterpret_cast<float4 *>(f)[((size_t)blockIdx.x * 6 + row) * 32 + lane] = make_float4((float)a.x, (float)a.y, (float)b.x, (float)b.y);
+    }
 }
 
-template <typename CT, typename R> __global__ void reorder_out_kernel(Geom g, CT *canon, const typename Vec<R>::T *__restrict__ even,
-                                                                      const typename Vec<R>::T *__restrict__ odd, int B)
+template <typename CT, typename R> __global__ void __launch_bounds__(RO_THREADS) reorder_out_kernel(Geom g, CT *canon, const typename Vec<R>::T *__restrict__ even,
+                                                                                                   const typename Vec<R>::T *__restrict__ odd, int B)
 {
-    const unsigned j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= (unsigned)g.Vh * B) return;
-    const int p = blockIdx.y, cb = j / B, rhs = j % B;
+    __shared__ double2 sm[12][33];
+    const int p = blockIdx.y;
     const long V = 2L * g.Vh;
-    typename CanonC<CT>::T *dst = reinterpret_cast<typename CanonC<CT>::T *>(canon) + ((long)rhs * V + lex_index(g, lex_of(g, cb, p))) * 12;
     const typename Vec<R>::T *f = p ? odd : even;
-    cx<R> psi[12];
-    if (f) load_spinor(f, j, psi);
-    else {
-#pragma unroll
-        for (int k = 0; k < 12; k++) psi[k] = mk<R>(0, 0);
+    {
+        const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;
+        if (!f) sm[row][lane] = make_double2(0., 0.);
+        else if (sizeof(R) == 8) sm[row][lane] = __ldg(reinterpret_cast<const double2 *>(f) + ((size_t)blockIdx.x * 12 + row) * 32 + lane);
+        else if (row < 6) {
+            const float4 v = __ldg(reinterpret_cast<const float4 *>(f) + ((size_t)blockIdx.x * 6 + row) * 32 + lane);
+            sm[2 * row][lane] = make_double2((double)v.x, (double)v.y);
+            sm[2 * row + 1][lane] = make_double2((double)v.z, (double)v.w);
+        }
     }
-#pragma unroll
-    for (int k = 0; k < 12; k++) {
-        typename CanonC<CT>::T v;
-        v.x = (CT)psi[k].re;
-        v.y = (CT)psi[k].im;
-        dst[k] = v;
-    }
+    __syncthreads();
+    const int chunk = threadIdx.x / 12, k = threadIdx.x % 12;
+    const unsigned j = blockIdx.x * 32u + chunk;
+    if (j >= (unsigned)g.Vh * B) return;
+    const int cb = j / B, rhs = j % B;
+    const double2 v = sm[k][chunk];
+    typename CanonC<CT>::T e;
+    e.x = (CT)v.x;
+    e.y = (CT)v.y;
+    reinterpret_cast<typename CanonC<CT>::T *>(canon)[((long)rhs * V + lex_index(g, lex_of(g, cb, p))) * 12 + k] = e;
 }
 
 template <typename CT, typename R>
 int reorder_in(const Geom &g, const CT *canon, typename Vec<R>::T *even, typename Vec<R>::T *odd, int B, cudaStream_t st)
 {
-    const unsigned n = (unsigned)g.Vh * B;
-    dim3 grid((n + 127) / 128, 2);
-    reorder_in_kernel<CT, R><<<grid, 128, 0, st>>>(g, canon, even, odd, B);
+    dim3 grid(lb_blocks((unsigned)g.Vh * B), 2);
+    reorder_in_kernel<CT, R><<<grid, RO_THREADS, 0, st>>>(g, canon, even, odd, B);
     CLV_CUDA(cudaGetLastError());
     return 0;
 }
@@ -298,9 +316,8 @@ int reorder_in(const Geom &g, const CT *canon, typename Vec<R>::T *even, typenam
 template <typename CT, typename R>
 int reorder_out(const Geom &g, CT *canon, const typename Vec<R>::T *even, const typename Vec<R>::T *odd, int B, cudaStream_t st)
 {
-    const unsigned n = (unsigned)g.Vh * B;
-    dim3 grid((n + 127) / 128, 2);
-    reorder_out_kernel<CT, R><<<grid, 128, 0, st>>>(g, canon, even, odd, B);
+    dim3 grid(lb_blocks((unsigned)g.Vh * B), 2);
+    reorder_out_kernel<CT, R><<<grid, RO_THREADS, 0, st>>>(g, canon, even, odd, B);
     CLV_CUDA(cudaGetLastError());
     return 0;
 }
