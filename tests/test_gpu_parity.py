@@ -200,3 +200,21 @@ def test_zero_source_and_errors(B):
     with pytest.raises(B.CloverError):
         B.Clover(dev(S.U), 0.12, 1.0, recon=8)
     S.ctx.close()
+
+
+def test_solve_is_deterministic_and_reports_max_iter(B):
+    """Reductions are summed in a fixed order (no atomics on data): two solves of the same sources agree bit for bit.  A solve cut
+    off by max_iter reports status 1 for every unfinished source, returns its best iterate and the true residual of that iterate."""
+    c = wl.CONFIGS[1]
+    S = Setup(B, c["dims"], c["eps"], c["kappa"], c["csw"], c["gauge_seed"])
+    eta = B.noise_fill(c["dims"], c["noise_seed"], 8, scale=wl.INV_SQRT2)
+    psi1, infos1, bad1 = S.ctx.solve(eta, tol=wl.TOL, batch=8, mixed=True)
+    psi2, infos2, bad2 = S.ctx.solve(eta, tol=wl.TOL, batch=8, mixed=True)
+    assert bad1 == bad2 == 0 and torch.equal(psi1, psi2) and infos1 == infos2
+    psi3, infos3, bad3 = S.ctx.solve(eta, tol=wl.TOL, batch=8, mixed=True, max_iter=5)
+    assert bad3 == 8 and all(i["status"] == 1 and i["iters"] == 5 for i in infos3)
+    e, p3 = eta.cpu().numpy(), psi3.cpu().numpy()
+    for r in (0, 7):
+        res = np.linalg.norm(e[r] - oracle.apply_D(S.U, S.A, S.bc, S.kappa, p3[r])) / np.linalg.norm(e[r])
+        assert 1e-10 < res < 1e-1 and abs(infos3[r]["true_resid"] - res) <= 1e-6 * res
+    S.ctx.close()
