@@ -121,6 +121,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--recon", type=int, default=0, choices=[0, 12, 18], help="override the workload's link storage of the fp32 operator (0: as configured)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel-bench", action="store_true", help="only time the three Dslash kernels alone (fp32/fp64, B = 1 and batch) and print them")
@@ -130,7 +131,9 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     from paper_1405_4524_b200 import workloads as wl
-    cfg = wl.CONFIGS[args.config]
+    cfg = dict(wl.CONFIGS[args.config])
+    if args.recon:
+        cfg["recon"] = args.recon
     if args.impl == "reference":
         return run_reference(args, cfg)
 
