@@ -390,7 +390,7 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, (sizeof(R) == 8 ? CLV_DSLASH_MIN
 #pragma unroll
                 for (int i = 0; i < 12; i++) f[i] = mk<float>((float)acc[i].re, (float)acc[i].im);
                 store_spinor(a.out32, j, f);
-            } else store_spinor(a.out, j, acc);
+            } else if (a.out) store_spinor(a.out, j, acc);   // neither: only the norm is wanted (final verification)
         } else store_spinor(a.out, j, acc);
         if (DOT == DOT_W) {
             cx<R> w[12];

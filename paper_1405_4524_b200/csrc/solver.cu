@@ -80,7 +80,8 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
             CLV_CUDA(cudaMemset(W->f64[i], 0, n64 * sizeof(double2)));
         }
         cudaFree(W->partial);
-        W->partial_blocks = std::max<int>(((unsigned)g.Vh * B + dslash_block_size() - 1) / dslash_block_size(), 148 * 8);
+        // twice the blocks of one Dslash launch: the final verification reduces the partials of two launches (even + odd) at once
+        W->partial_blocks = 2 * std::max<int>(((unsigned)g.Vh * B + dslash_block_size() - 1) / dslash_block_size(), 148 * 8);
         CLV_CUDA(cudaMalloc(&W->partial, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
         CLV_CUDA(cudaMemset(W->partial, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
         if (!W->sc_dev) {
@@ -229,7 +230,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         CLV_CUDA(cudaEventRecord(W->ev_dep, st_user));
         CLV_CUDA(cudaStreamWaitEvent(st, W->ev_dep, 0));
     }
-    double2 *eta_e = W->f64[F_ETA_E], *eta_o = W->f64[F_ETA_O], *b = W->f64[F_B], *y = W->f64[F_Y], *r64 = W->f64[F_R64], *w64 = W->f64[F_W64],
+    double2 *eta_e = W->f64[F_ETA_E], *eta_o = W->f64[F_ETA_O], *b = W->f64[F_B], *y = W->f64[F_Y], *r64 = W->f64[F_R64],
             *tmp64 = W->f64[F_TMP64], *psi_o = W->f64[F_PSI_O];
     V *x = (V *)W->sl[S_X], *r = (V *)W->sl[S_R], *p = (V *)W->sl[S_P], *v = (V *)W->sl[S_V], *s = (V *)W->sl[S_S], *t = (V *)W->sl[S_T],
       *r0 = (V *)W->sl[S_R0], *tmp = (V *)W->sl[S_TMP];
@@ -351,13 +352,18 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         }
     }
     CLV_CUDA(cudaEventRecord(W->ev[3], st));
-    // odd sites and verification on the full lattice, all fp64
+    // odd sites and verification on the full lattice, all fp64: ||eta - D psi||^2 comes out of the epilogues of the two Dslash
+    // launches that apply D (residual variant without a store), their per-block partials reduced together
     CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, eta_o, psi_o, ctx->kappa, 1, XM_PLAIN, 1), B, st, nullptr));
-    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(psi_o, y, w64, -ctx->kappa, 0, XM_CLOVER, 0), B, st, nullptr));
-    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, psi_o, tmp64, -ctx->kappa, 1, XM_CLOVER, 0), B, st, nullptr));
+    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(psi_o, y, nullptr, -ctx->kappa, 0, XM_CLOVER, 0, DOT_RES, eta_e, W->partial), B, st, &grid));
+    if (2 * grid > W->partial_blocks) {
+        set_error("solve: partial buffer too small for the verification (%d blocks)", grid);
+        return CLOVER_EINVAL;
+    }
+    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, psi_o, nullptr, -ctx->kappa, 1, XM_CLOVER, 0, DOT_RES, eta_o, W->partial + (size_t)grid * B * 4), B, st,
+                                    nullptr));
     nl += 3;
-    CLV_CHECK(blas_norm2_pair(bc, eta_e, w64, eta_o, tmp64, &nb));
-    CLV_CHECK(blas_scalar_step(bc, SC_FINAL, nb, tol2, delta2));
+    CLV_CHECK(blas_scalar_step(bc, SC_FINAL, 2 * grid, tol2, delta2));
     CLV_CUDA(cudaEventRecord(W->ev[4], st));
     CLV_CHECK((reorder_out<double, double>(g, dst, y, psi_o, B, st)));
     nl++;
