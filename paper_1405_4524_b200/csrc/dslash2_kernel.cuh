@@ -81,6 +81,9 @@ __device__ __forceinline__ void hop_load2(const Geom &g, const OpData<float> &op
 #else
     load_spinor2(in, (unsigned)nb * B + rhs, d.psiA, d.psiB);
 #endif
+#ifdef CLV_ABL_TGAUGE
+    if (MU == 3) { d.neg = wrap && g.bc[MU] < 0; return; }   // timing of a temporal-gauge hop: no t link at all
+#endif
 #ifdef CLV_ABL_NOLINK
 #pragma unroll
     for (int i = 0; i < 9; i++) d.u[i] = mk<float>(__int_as_float(0x3f000000 + (cb >> 3) + i + 16 * MU), __int_as_float(0x3e800000 + i + FWD));
@@ -119,6 +122,13 @@ template <int RECON, int MU, int FWD> __device__ __forceinline__ void hop_comput
             hB[i] = mk<float>(-hB[i].re, -hB[i].im);
         }
     }
+#ifdef CLV_ABL_TGAUGE
+    if (MU == 3) {
+        accA.template add_unit_t<FWD>(hA);
+        accB.template add_unit_t<FWD>(hB);
+        return;
+    }
+#endif
     accA.template add<MU, FWD>(hA, d.u);
     accB.template add<MU, FWD>(hB, d.u);
 }

@@ -160,6 +160,19 @@ template <> struct HopAcc<float> {
             }
         }
     }
+    // mu = t with a unit link (temporal gauge): g = h, no SU(3) product
+    template <int FWD> __device__ __forceinline__ void add_unit_t(const cx<float> h[6])
+    {
+        constexpr float s = FWD ? -1.f : 1.f;
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            const float2 gre = make_float2(h[a].re, h[3 + a].re), gim = make_float2(h[a].im, h[3 + a].im);
+            ure[a] = __fadd2_rn(ure[a], gre);
+            uim[a] = __fadd2_rn(uim[a], gim);
+            lre[a] = __ffma2_rn(gre, make_float2(s, s), lre[a]);
+            lim[a] = __ffma2_rn(gim, make_float2(s, s), lim[a]);
+        }
+    }
     __device__ __forceinline__ void finish(cx<float> out[12]) const
     {
 #pragma unroll
