@@ -15,6 +15,9 @@ namespace clv {
 #ifndef CLV_R2_MINB
 #define CLV_R2_MINB 3
 #endif
+#ifndef CLV_R2_BLOCK_NODOT
+#define CLV_R2_BLOCK_NODOT 32   // threads per CTA of the pair-kernel variants without dot products
+#endif
 #ifndef CLV_R2_SMEM
 #define CLV_R2_SMEM 1   // stage the CTA's clover blocks in shared memory with cp.async at kernel start
 #endif
@@ -227,15 +230,19 @@ template <int DOT> __device__ __forceinline__ void dots(const cx<float> acc[12],
     }
 }
 
-template <int B, int RECON, int XMODE, int PINV, int DOT>
-__global__ void __launch_bounds__(DSLASH_BLOCK, CLV_R2_MINB) dslash2_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
+// BLOCK threads per CTA, the register budget of 12 resident warps per SM whatever BLOCK is.  One-warp CTAs retire and refill
+// the SM at a finer grain (A^-1 H: 225 -> 211 us at 24^3x48); variants with dot products keep 128 threads, because every CTA
+// writes a line of partial sums that the scalar kernel must read back (four times as many CTAs cost more than they gain).
+template <int B, int RECON, int XMODE, int PINV, int DOT, int BLOCK>
+__global__ void __launch_bounds__(BLOCK, CLV_R2_MINB * DSLASH_BLOCK / BLOCK)
+dslash2_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
 {
     static_assert(B >= 2 && B % 2 == 0, "pairs of right-hand sides");
-    const unsigned j = 2u * (blockIdx.x * DSLASH_BLOCK + threadIdx.x);   // first rhs of this thread's pair
+    const unsigned j = 2u * (blockIdx.x * BLOCK + threadIdx.x);   // first rhs of this thread's pair
     const bool active = j < (unsigned)g.Vh * B;
     double dA[3] = {0, 0, 0}, dB[3] = {0, 0, 0};
     const int p = a.parity;
-    constexpr int SITES = 2 * DSLASH_BLOCK / B;   // sites of this CTA: consecutive cb from blockIdx.x * SITES
+    constexpr int SITES = 2 * BLOCK / B;   // sites of this CTA: consecutive cb from blockIdx.x * SITES
     __shared__ __align__(16) float4 cl_s[(CLV_R2_SMEM && (XMODE == XM_CLOVER || PINV)) ? SITES * 18 : 1];
     if (CLV_R2_SMEM && (XMODE == XM_CLOVER || PINV)) {
         // the one clover field this variant needs (A for X = A x, A^-1 for P): 288 bytes per site, 16-byte async copies whose
@@ -243,7 +250,7 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, CLV_R2_MINB) dslash2_kernel(cons
         const float2 *clov = PINV ? (p ? op.clov_inv[1] : op.clov_inv[0]) : (p ? op.clov[1] : op.clov[0]);
         const float4 *base4 = reinterpret_cast<const float4 *>(clov);
         const unsigned cb0 = blockIdx.x * SITES;
-        for (int item = threadIdx.x; item < SITES * 18; item += DSLASH_BLOCK) {
+        for (int item = threadIdx.x; item < SITES * 18; item += BLOCK) {
             const int row = item / SITES, site = item % SITES;
             const unsigned cbs = cb0 + site;
             if (cbs < (unsigned)g.Vh) __pipeline_memcpy_async(&cl_s[site * 18 + row], base4 + ((size_t)(cbs >> 5) * 18 + row) * 32 + (cbs & 31u), 16);
@@ -314,7 +321,7 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, CLV_R2_MINB) dslash2_kernel(cons
         dots<DOT>(accA, xA, wA, dA);
         dots<DOT>(accB, xB, wB, dB);
     }
-    if (DOT != DOT_NONE) block_reduce_pair<B, DSLASH_BLOCK>(dA, dB, a.partial);
+    if (DOT != DOT_NONE) block_reduce_pair<B, BLOCK>(dA, dB, a.partial);
 }
 
 }  // namespace clv
