@@ -64,12 +64,13 @@ static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const Ds
     if (PairLaunch<R, B, RECON>::use() && (a.xmode != XM_NONE || a.pinv)) return PairLaunch<R, B, RECON>::go(ctx, op, a, st, grid_out);
     const Geom &g = ctx->geom;
     const unsigned n = (unsigned)g.Vh * B;
-    const unsigned grid = (n + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
+    const unsigned block = a.dot == DOT_NONE ? CLV_DSLASH_BLOCK_NODOT : DSLASH_BLOCK;
+    const unsigned grid = (n + block - 1) / block;
     if (grid_out) *grid_out = (int)grid;
     const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
 #define CLV_LAUNCH(XM, PI, DT)                                                          \
     case (XM) * 100 + (PI) * 10 + (DT):                                                 \
-        dslash_kernel<R, B, RECON, XM, PI, DT><<<grid, DSLASH_BLOCK, 0, st>>>(g, op, a); \
+        dslash_kernel<R, B, RECON, XM, PI, DT, ((DT) == DOT_NONE ? CLV_DSLASH_BLOCK_NODOT : DSLASH_BLOCK)><<<grid, block, 0, st>>>(g, op, a); \
         break;
     switch (key) {
         CLV_LAUNCH(XM_NONE, 0, DOT_NONE)
