@@ -15,3 +15,12 @@ import numpy as np
 def timeslice_norm2(f, n_outer, T):
     f = np.asarray(f, dtype=np.complex128).reshape(n_outer, T, -1)
     return np.sum(f.real ** 2 + f.imag ** 2, axis=(0, 2))
+
+
+def timeslice_inner(a, b, n_outer, T):
+    """out[t] = sum_{o, k} a[o, t, k] conj(b[o, t, k]): with a, b two fills of eq. 7.3 from INDEPENDENT source sets this is
+    sum_x sum_z Tr[S_s^(1)(t,z;0,x) S_s^(2)dagger(t,z;0,x)], the paper's "two sets of random sources, one for S and one for
+    S^dagger" (PAPER.md L303), whose point (Figs. 2-3, L312-316) is that it has no noise-squared bias; a = b gives timeslice_norm2."""
+    a = np.asarray(a, dtype=np.complex128).reshape(n_outer, T, -1)
+    b = np.asarray(b, dtype=np.complex128).reshape(n_outer, T, -1)
+    return np.sum(a * np.conj(b), axis=(0, 2))
