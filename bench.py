@@ -337,6 +337,18 @@ def main():
         c1.record()
         torch.cuda.synchronize()
         t_trace = c0.elapsed_time(c1) / 3 * 1e-3
+        # the two-source-set trace: a second fill from an independent noise set, then sum Tr[S1 S2^+] per timeslice
+        fs2 = torch.empty_like(fs)
+        B.stochastic_fill(B.noise_fill(fd, 978, n_rhs, scale=1.0), B.noise_fill(fd, 2002, n_rhs, scale=wl.INV_SQRT2), t0=0, scale=wl.INV_SQRT2, out=fs2)
+        B.timeslice_inner(fs, fs2, 1, 16)
+        torch.cuda.synchronize()
+        c0.record()
+        for _ in range(3):
+            B.timeslice_inner(fs, fs2, 1, 16)
+        c1.record()
+        torch.cuda.synchronize()
+        t_inner = c0.elapsed_time(c1) / 3 * 1e-3
+        del fs2
         fbytes = fs.numel() * 16
         fflop = 8.0 * fs.numel() * n_rhs
         fp64_peak = 148 * 64 * 2 * 1.965e9
@@ -347,6 +359,8 @@ def main():
                     "trace": {"what": "sum_x sum_z Tr S_s S_s^+ for all 16 timeslices (Table I last row)", "ms": t_trace * 1e3,
                               "read_gbs": fbytes / t_trace / 1e9, "frac_hbm": fbytes / t_trace / 1e9 / peaks["hbm_gbs"],
                               "paper_table1_s_per_timeslice": 43.3},
+                    "trace_two_sets": {"what": "sum_x sum_z Tr S_s1 S_s2^+ for all 16 timeslices, fills from two independent source sets (P:L303)",
+                                       "ms": t_inner * 1e3, "read_gbs": 2 * fbytes / t_inner / 1e9, "frac_hbm": 2 * fbytes / t_inner / 1e9 / peaks["hbm_gbs"]},
                     "paper_table2_s_per_source": {"cpu": 100.8, "gpu": 8.8, "hardware": "unnamed", "cite": "PAPER.md L340-344"}}
         del fs, fe, fx
 

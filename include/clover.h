@@ -129,6 +129,11 @@ int stochastic_fill(const double *x_dev, const double *eta_dev, const int dims[4
  * zero-momentum pion correlator; with f = the array of stochastic_fill (n_outer = 1, slice_len = 144 L^6) it is
  * sum_x sum_z Tr[S_s(t,z;0,x) S_s^+(t,z;0,x)].  out_dev: double [T] (device).  fp64, deterministic.  Asynchronous on `stream`. */
 int timeslice_norm2(const double *f_dev, long long n_outer, int T, long long slice_len, double *out_dev, void *stream);
+/* out[t] = sum_{o, k} a[o][t][k] conj(b[o][t][k]) for two complex128 device fields of that shape: with a, b the arrays of two
+ * stochastic_fill calls fed from INDEPENDENT source sets ("two sets of random sources, one for S and one for S^+", P:L303;
+ * Figs. 2-3: no noise-squared bias, unlike the one-set trace) this is sum_x sum_z Tr[S_s^(1) S_s^(2)+](t).
+ * out_dev: double [T][2] (device).  a_dev = b_dev gives (timeslice_norm2, 0).  fp64, deterministic.  Asynchronous on `stream`. */
+int timeslice_inner(const double *a_dev, const double *b_dev, long long n_outer, int T, long long slice_len, double *out_dev, void *stream);
 
 /* ---- measurement helpers (internal layout, no reorders; used by bench.py and the ncu runs) ---- */
 enum {

@@ -18,7 +18,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 OP_HOP_EO, OP_HOP_OE, OP_HOP_FULL, OP_CLOVER, OP_CLOVER_INV, OP_D_FULL, OP_MHAT = range(7)
 KERNEL_HOP, KERNEL_AINV_HOP, KERNEL_A_MINUS_HOP = range(3)
 EXPORTS = ["clover_create", "clover_destroy", "dslash_apply", "clover_solve", "clover_solve_host", "noise_fill",
-           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill", "timeslice_norm2"]
+           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill", "timeslice_norm2", "timeslice_inner"]
 
 
 class ClovOpts(ctypes.Structure):
@@ -52,6 +52,7 @@ _lib.stochastic_operators.argtypes = [_vp, _vp, _ip, _i, _vp, _vp]
 _lib.stochastic_correlator.argtypes = [_vp, _i, _i, _d, _vp, _vp]
 _lib.stochastic_fill.argtypes = [_vp, _vp, _ip, _i, _i, _d, _i, _vp, _vp]
 _lib.timeslice_norm2.argtypes = [_vp, ctypes.c_longlong, _i, ctypes.c_longlong, _vp, _vp]
+_lib.timeslice_inner.argtypes = [_vp, _vp, ctypes.c_longlong, _i, ctypes.c_longlong, _vp, _vp]
 _lib.clover_last_error.restype = ctypes.c_char_p
 
 
@@ -139,6 +140,17 @@ def timeslice_norm2(f, n_outer, T):
     assert f.is_cuda and f.is_contiguous() and f.dtype == torch.complex128 and f.numel() % (n_outer * T) == 0
     out = torch.empty(T, dtype=torch.float64, device="cuda")
     _check(_lib.timeslice_norm2(f.data_ptr(), n_outer, T, f.numel() // (n_outer * T), out.data_ptr(), _stream()))
+    return out
+
+
+def timeslice_inner(a, b, n_outer, T):
+    """out[t] = sum a[o, t, :] conj(b[o, t, :]) for two complex128 device tensors viewed as [n_outer, T, -1]: the trace between
+    fills from two independent source sets."""
+    _require_cuda()
+    assert a.is_cuda and a.is_contiguous() and a.dtype == torch.complex128 and a.numel() % (n_outer * T) == 0
+    assert b.is_cuda and b.is_contiguous() and b.dtype == torch.complex128 and b.numel() == a.numel()
+    out = torch.empty(T, dtype=torch.complex128, device="cuda")
+    _check(_lib.timeslice_inner(a.data_ptr(), b.data_ptr(), n_outer, T, a.numel() // (n_outer * T), out.data_ptr(), _stream()))
     return out
 
 

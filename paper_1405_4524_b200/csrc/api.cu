@@ -155,6 +155,14 @@ int timeslice_norm2(const double *f_dev, long long n_outer, int T, long long sli
     return launch_timeslice_norm2(f_dev, (long)n_outer, T, (long)slice_len, out_dev, (cudaStream_t)stream);
 }
 
+int timeslice_inner(const double *a_dev, const double *b_dev, long long n_outer, int T, long long slice_len, double *out_dev, void *stream)
+{
+    if (!a_dev || !b_dev || !out_dev) { set_error("timeslice_inner: null argument"); return CLOVER_EINVAL; }
+    if (n_outer < 1 || T < 1 || T > 65535 || slice_len < 1) { set_error("timeslice_inner: bad n_outer, T or slice_len"); return CLOVER_EINVAL; }
+    CLV_CHECK(check_device());
+    return launch_timeslice_inner(a_dev, b_dev, (long)n_outer, T, (long)slice_len, out_dev, (cudaStream_t)stream);
+}
+
 int clover_bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms_per_launch, void *stream)
 {
     if (!ctx || !ms_per_launch) { set_error("clover_bench_kernel: null argument"); return CLOVER_EINVAL; }

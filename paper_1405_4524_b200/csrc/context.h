@@ -93,6 +93,7 @@ int launch_fill(const double *x, const double *eta, const int dims[4], int n, in
 
 // ---- traces.cu ----
 int launch_timeslice_norm2(const double *f, long n_outer, int T, long slice_len, double *out, cudaStream_t st);
+int launch_timeslice_inner(const double *a, const double *b, long n_outer, int T, long slice_len, double *out, cudaStream_t st);
 
 // ---- solver.cu ----
 int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, double tol, int max_iter, int batch, int mixed,

@@ -21,6 +21,21 @@ def test_timeslice_norm2(n_outer, T, L):
     assert np.abs(got - want).max() / np.abs(want).max() < 1e-13
 
 
+@pytest.mark.parametrize("n_outer,T,L", [(1, 4, 7), (12, 8, 768), (3, 16, 100003), (2, 2, 1)])
+def test_timeslice_inner(n_outer, T, L):
+    from paper_1405_4524_b200 import binding as B
+    rng = np.random.default_rng(6)
+    a = rng.standard_normal((n_outer, T, L)) + 1j * rng.standard_normal((n_outer, T, L))
+    b = rng.standard_normal((n_outer, T, L)) + 1j * rng.standard_normal((n_outer, T, L))
+    ad, bd = torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda()
+    got = B.timeslice_inner(ad, bd, n_outer, T).cpu().numpy()
+    want = traces.timeslice_inner(a, b, n_outer, T)
+    scale = np.sqrt(traces.timeslice_norm2(a, n_outer, T) * traces.timeslice_norm2(b, n_outer, T)).max()
+    assert np.abs(got - want).max() / scale < 1e-13
+    same = B.timeslice_inner(ad, ad, n_outer, T).cpu().numpy()
+    assert np.abs(same.imag).max() == 0.0 and np.abs(same.real - traces.timeslice_norm2(a, n_outer, T)).max() / scale < 1e-13
+
+
 def test_point_and_stochastic_pion_correlators_on_4x4x4x8():
     """compare stochastic propagators with exact point-source ones on a lattice small enough.  The whole
     pipeline runs on the device: 12 point solves -> sum_y Tr S_p S_p^+ ; noise -> solves -> fill -> sum_x sum_z Tr S_s S_s^+."""
@@ -60,4 +75,13 @@ def test_point_and_stochastic_pion_correlators_on_4x4x4x8():
     assert np.all(signal > 0)
     assert 0.5 < signal[0] / Cp[0] < 2.0 and 0.3 < signal[T // 2] / Cp[T // 2] < 3.0
     assert Cp[0] > Cp[1] > Cp[2] and signal[0] > signal[1] > signal[2]
+    # the paper's other option (L303, Figs. 2-3): S and S^+ from two independent source sets -- no noise floor to subtract
+    S1 = B.stochastic_fill(psi[:256].contiguous(), eta[:256].contiguous(), t0=0, scale=wl.INV_SQRT2)
+    S2 = B.stochastic_fill(psi[256:].contiguous(), eta[256:].contiguous(), t0=0, scale=wl.INV_SQRT2)
+    two = B.timeslice_inner(S1, S2, 1, T).cpu().numpy() / V3
+    want = traces.timeslice_inner(S1.cpu().numpy(), S2.cpu().numpy(), 1, T) / V3
+    assert np.abs(two - want).max() / np.abs(want).max() < 1e-12
+    for t in range(3):
+        assert 0.6 < two[t].real / signal[t] < 1.6 and abs(two[t].imag) < 0.3 * signal[t]
+        assert Cs[128][t] > 2 * two[t].real          # the one-set trace carries the (n-1)/N_r noise-squared bias
     ctx.close()
