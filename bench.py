@@ -184,7 +184,7 @@ def main():
     eta = torch.empty((n_rhs, T, Z, Y, X, 4, 3), dtype=torch.complex128, device="cuda")
     psi = torch.empty_like(eta)
     launches = 0
-    kstats = {"n_ainv_hop": 0, "n_a_minus_hop": 0, "ms_ainv_hop": 0.0, "ms_a_minus_hop": 0.0}
+    kstats = {"n_ainv_hop": 0, "n_a_minus_hop": 0, "ms_ainv_hop": 0.0, "ms_a_minus_hop": 0.0, "n_a_minus_hop_s": 0, "ms_a_minus_hop_s": 0.0}
     phases = {k: 0.0 for k in ("ms_total", "ms_reorder", "ms_prep", "ms_iterate", "ms_reliable", "ms_finish")}
     last = {}
 
@@ -222,7 +222,8 @@ def main():
     peaks, peak_kind = measured_peaks()
     b = 4 if cfg["mixed"] else 8
     g = cfg["recon"] if cfg["mixed"] else 18
-    bytes_a_minus = (8 * g * b + 72 * b) / batch + 24 * b * 3          # links + clover shared by the batch; in, x, out per rhs
+    merged = kstats["n_a_minus_hop_s"] > 0   # merged iteration (solver.cu): both fused Dslash variants also read w (r or r0) at the own site
+    bytes_a_minus = (8 * g * b + 72 * b) / batch + 24 * b * (4 if merged else 3)   # links + clover shared by the batch; in, x, (w,) out per rhs
     bytes_ainv = (8 * g * b + 72 * b) / batch + 24 * b * 2
     prec = 32 if cfg["mixed"] else 64
     timed = "CUDA events around every launch inside the timed steps"
@@ -238,14 +239,20 @@ def main():
     tp = os.path.join(ROOT, "profiles", "traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
         traffic = json.load(open(tp)).get(f"a_minus_hop_{cfg['name']}_b{batch}")
-    roofline = {"bound": "hbm", "kernel": (f"dslash2_kernel<B={batch},recon={g},A x - k^2 H t,+dots> (fp32, one thread per site and rhs pair)" if cfg["mixed"] and batch >= 2
-                           else f"dslash_kernel<{'float' if cfg['mixed'] else 'double'},B={batch},recon={g},A x - k^2 H t,+dots>"),
+    epi = "t = A s - k^2 H tmp, +<t,s>,<t,t>,<r0,t>,<r0,s>" if merged else "A x - k^2 H t,+dots"
+    roofline = {"bound": "hbm", "kernel": (f"dslash2_kernel<B={batch},recon={g},{epi}> (fp32, one thread per site and rhs pair)" if cfg["mixed"] and batch >= 2
+                           else f"dslash_kernel<{'float' if cfg['mixed'] else 'double'},B={batch},recon={g},{epi}>"),
                 "achieved": ach, "timed": timed, "peak": peaks["hbm_gbs"], "peak_kind": peak_kind, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                 "traffic": traffic, "algorithmic_bytes_per_site_rhs": bytes_a_minus, "us_per_launch": t_a_minus * 1e6,
                 "gflops": 1872.0 * Vh * batch / t_a_minus / 1e9,
                 "other_kernels": {"ainv_hop": {"achieved": bytes_ainv * Vh * batch / t_ainv / 1e9, "us_per_launch": t_ainv * 1e6,
                                                "frac": bytes_ainv * Vh * batch / t_ainv / 1e9 / peaks["hbm_gbs"],
                                                "algorithmic_bytes_per_site_rhs": bytes_ainv}}}
+    if merged:   # the other fused variant of the iteration: s = r - alpha (A p - k^2 H tmp), same bytes, no reduction
+        t_s = kstats["ms_a_minus_hop_s"] / kstats["n_a_minus_hop_s"] * 1e-3
+        roofline["other_kernels"]["a_minus_hop_s"] = {"achieved": bytes_a_minus * Vh * batch / t_s / 1e9, "us_per_launch": t_s * 1e6,
+                                                      "frac": bytes_a_minus * Vh * batch / t_s / 1e9 / peaks["hbm_gbs"],
+                                                      "algorithmic_bytes_per_site_rhs": bytes_a_minus}
 
     # ---- the plain Wilson hop kernel timed alone (BASELINE.json: "clover Dslash GB/s"), fields larger than L2 or L2 flushed ----
     dslash = {}

@@ -157,6 +157,10 @@ typedef struct {
        ainv_hop = t_o = A_oo^-1 H_oe x_e ;  a_minus_hop = y_e = A_ee x_e - kappa^2 H_eo t_o with its dot-product epilogue */
     long long n_ainv_hop, n_a_minus_hop;
     double ms_ainv_hop, ms_a_minus_hop;
+    /* merged iteration (default): the a_minus_hop launch of Mhat p that also writes s = r - alpha v is counted here, and
+       n_a_minus_hop / ms_a_minus_hop count the one of Mhat s (with <t,s>, <t,t>, <r0,t>, <r0,s>) */
+    long long n_a_minus_hop_s;
+    double ms_a_minus_hop_s;
 } clover_solve_stats;
 int clover_get_stats(const clover_ctx *ctx, clover_solve_stats *out);
 

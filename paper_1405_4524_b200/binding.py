@@ -34,7 +34,8 @@ class SolveStats(ctypes.Structure):
     _fields_ = [("kernel_launches", ctypes.c_longlong), ("ms_total", ctypes.c_double), ("ms_reorder", ctypes.c_double),
                 ("ms_prep", ctypes.c_double), ("ms_iterate", ctypes.c_double), ("ms_reliable", ctypes.c_double),
                 ("ms_finish", ctypes.c_double), ("n_ainv_hop", ctypes.c_longlong), ("n_a_minus_hop", ctypes.c_longlong),
-                ("ms_ainv_hop", ctypes.c_double), ("ms_a_minus_hop", ctypes.c_double)]
+                ("ms_ainv_hop", ctypes.c_double), ("ms_a_minus_hop", ctypes.c_double), ("n_a_minus_hop_s", ctypes.c_longlong),
+                ("ms_a_minus_hop_s", ctypes.c_double)]
 
 
 _vp, _ip, _i, _d = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.c_int, ctypes.c_double

@@ -104,10 +104,14 @@ __global__ void __launch_bounds__(BLAS_BLOCK) xr_update_kernel(size_t n, int B, 
 
 // ---- r0 = r for the rhs flagged `restart` ------------------------------------------------------------
 template <typename V> __global__ void __launch_bounds__(BLAS_BLOCK) restart_kernel(size_t n, int B, const RhsScalars *__restrict__ sc, const V *__restrict__ r,
-                                                                                    V *__restrict__ r0)
+                                                                                    V *__restrict__ r0, V *__restrict__ p)
 {
-    if (!sc[threadIdx.x & (B - 1)].restart) return;
-    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) r0[i] = r[i];
+    if (sc[threadIdx.x & (B - 1)].restart != 1) return;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        const V a = r[i];
+        r0[i] = a;
+        if (p) p[i] = a;   // merged iteration: the search direction restarts with the shadow residual
+    }
 }
 
 // ---- p = r + beta (p - omega v) ---------------------------------------------------------------------
@@ -117,6 +121,55 @@ template <typename V> __global__ void __launch_bounds__(BLAS_BLOCK) p_update_ker
     const RhsScalars &q = sc[threadIdx.x & (B - 1)];
     const zs be = ld_z(q.beta), mom = neg(ld_z(q.omega));
     for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) p[i] = caxpy(be, caxpy(mom, v[i], p[i]), r[i]);
+}
+
+// ---- merged iteration (solver.cu): x += alpha p + omega s ; r' = s - omega t ; p = r' + beta p - gam (r - s) ; <q0,p>, ||r'||^2.
+//      (r - s = alpha v and gam = beta omega / alpha, so this is p = r' + beta (p - omega v) without v ever being stored.) ----
+__device__ __forceinline__ float4 vsub(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
+__device__ __forceinline__ double2 vsub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+template <typename V>
+__global__ void __launch_bounds__(BLAS_BLOCK) xrp_update_kernel(size_t n, int B, const RhsScalars *__restrict__ sc, V *__restrict__ x, V *__restrict__ r,
+                                                                V *__restrict__ p, const V *__restrict__ s, const V *__restrict__ t,
+                                                                const V *__restrict__ q0, double *__restrict__ partial)
+{
+    const RhsScalars &q = sc[threadIdx.x & (B - 1)];
+    const zs al = ld_z(q.alpha), om = ld_z(q.omega), mom = neg(om), be = ld_z(q.beta), mga = neg(ld_z(q.gam));
+    double d0 = 0, d1 = 0, d2 = 0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        const V sv = s[i], pv = p[i], ro = r[i];
+        x[i] = caxpy(om, sv, caxpy(al, pv, x[i]));
+        const V rn = caxpy(mom, t[i], sv);
+        r[i] = rn;
+        const V pn = caxpy(mga, vsub(ro, sv), caxpy(be, pv, rn));
+        p[i] = pn;
+        cdot_acc(q0[i], pn, d0, d1);
+        d2 += norm2(rn);
+    }
+    block_reduce(B, d0, d1, d2, partial);
+}
+
+// ---- out = gamma5 in (chiral basis: spins 2, 3 change sign = the upper half of the NV vectors of an entry);
+//      `masked`: only the rhs flagged `restart == 1` are written ------------------------------------------------
+__device__ __forceinline__ float4 vneg(float4 a) { return make_float4(-a.x, -a.y, -a.z, -a.w); }
+__device__ __forceinline__ double2 vneg(double2 a) { return make_double2(-a.x, -a.y); }
+template <typename V, int NV>
+__global__ void __launch_bounds__(BLAS_BLOCK) gamma5_kernel(size_t n, int B, const RhsScalars *__restrict__ sc, int masked, const V *__restrict__ in,
+                                                            V *__restrict__ out)
+{
+    if (masked && sc[threadIdx.x & (B - 1)].restart != 1) return;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) {
+        const V a = in[i];
+        out[i] = ((i >> 5) % NV >= NV / 2) ? vneg(a) : a;
+    }
+}
+
+// ---- partial <a, b> -----------------------------------------------------------------------------------
+template <typename V>
+__global__ void __launch_bounds__(BLAS_BLOCK) cdot_kernel(size_t n, int B, const V *__restrict__ a, const V *__restrict__ b, double *__restrict__ partial)
+{
+    double d0 = 0, d1 = 0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_BLOCK) cdot_acc(a[i], b[i], d0, d1);
+    block_reduce(B, d0, d1, 0., partial);
 }
 
 // ---- y += x ; x = 0.  fp32 x: vector (jb, k, lane) holds the complex numbers 2k, 2k+1 = fp64 vectors (jb, 2k), (jb, 2k+1) ----
@@ -210,38 +263,42 @@ __device__ __forceinline__ bool finite_z(zs z) { return isfinite(z.re) && isfini
 
 // one block per rhs: sum partial[(b*B + rhs)*4 + c] over b < nblocks in a fixed order, then thread 0 updates the scalars.
 constexpr int SC_SLICES = 32;
-__global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblocks, const double *__restrict__ partial, RhsScalars *sc, double tol2,
-                                                     double delta2, double *stage, unsigned *ticket)
+__global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblocks, const double *__restrict__ partial, const double *__restrict__ partial2,
+                                                     RhsScalars *sc, double tol2, double delta2, double *stage, unsigned *ticket)
 {
-    __shared__ double sm[256][3];
+    __shared__ double sm[256][7];
     __shared__ bool last;
     const int rhs = blockIdx.x, slice = blockIdx.y;
-    // stage 1: this block sums its contiguous slice of the per-block partials (fixed order)
+    // stage 1: this block sums its contiguous slice of the per-block partials (fixed order); plane 2 only where the step has one
     const int per = (nblocks + SC_SLICES - 1) / SC_SLICES, lo = slice * per, hi = min(nblocks, lo + per);
-    double a0 = 0, a1 = 0, a2 = 0;
+    double a[7] = {0, 0, 0, 0, 0, 0, 0};
     for (int b = lo + threadIdx.x; b < hi; b += 256) {
         const double *q = partial + ((size_t)b * B + rhs) * 4;
-        a0 += q[0];
-        a1 += q[1];
-        a2 += q[2];
+        a[0] += q[0];
+        a[1] += q[1];
+        a[2] += q[2];
+        if (partial2) {
+            const double *q2 = partial2 + ((size_t)b * B + rhs) * 4;
+            a[3] += q2[0];
+            a[4] += q2[1];
+            a[5] += q2[2];
+            a[6] += q2[3];
+        }
     }
-    sm[threadIdx.x][0] = a0;
-    sm[threadIdx.x][1] = a1;
-    sm[threadIdx.x][2] = a2;
+#pragma unroll
+    for (int c = 0; c < 7; c++) sm[threadIdx.x][c] = a[c];
     __syncthreads();
     for (int s = 128; s > 0; s >>= 1) {
         if ((int)threadIdx.x < s) {
-            sm[threadIdx.x][0] += sm[threadIdx.x + s][0];
-            sm[threadIdx.x][1] += sm[threadIdx.x + s][1];
-            sm[threadIdx.x][2] += sm[threadIdx.x + s][2];
+#pragma unroll
+            for (int c = 0; c < 7; c++) sm[threadIdx.x][c] += sm[threadIdx.x + s][c];
         }
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        double *o = stage + ((size_t)rhs * SC_SLICES + slice) * 4;
-        o[0] = sm[0][0];
-        o[1] = sm[0][1];
-        o[2] = sm[0][2];
+        double *o = stage + ((size_t)rhs * SC_SLICES + slice) * 8;
+#pragma unroll
+        for (int c = 0; c < 7; c++) o[c] = sm[0][c];
         __threadfence();
         last = (atomicAdd(ticket + rhs, 1u) == SC_SLICES - 1);
     }
@@ -250,12 +307,16 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
     // stage 2 (last block of this rhs to arrive): sum the slices in order, then the scalar recurrences
     __threadfence();
     ticket[rhs] = 0;
-    double d0 = 0, d1 = 0, d2 = 0;
+    double d0 = 0, d1 = 0, d2 = 0, e0 = 0, e1 = 0, e2 = 0, e3 = 0;
     for (int k = 0; k < SC_SLICES; k++) {
-        const volatile double *o = stage + ((size_t)rhs * SC_SLICES + k) * 4;
+        const volatile double *o = stage + ((size_t)rhs * SC_SLICES + k) * 8;
         d0 += o[0];
         d1 += o[1];
         d2 += o[2];
+        e0 += o[3];
+        e1 += o[4];
+        e2 += o[5];
+        e3 += o[6];
     }
     RhsScalars &q = sc[rhs];
     const zs zero{0., 0.};
@@ -267,15 +328,17 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         q.want_update = 0;
         break;
     case SC_INIT:  // d0 = ||r||^2 with r = b_e (y = 0)
+    case SC_INIT_MERGED:
         q.rho = make_double2(d0, 0.);
         q.r2 = q.maxr2 = q.true_r2 = d0;
-        q.alpha = q.omega = q.beta = make_double2(0., 0.);
+        q.alpha = q.omega = q.beta = q.gam = make_double2(0., 0.);
         q.want_update = 0;
         q.claim = 0;
         q.restart = 0;
         q.nrestart = 0;
         if (!(q.eta2 > 0.) || d0 <= tol2 * q.eta2) q.done = 1;  // zero source or already converged
         if (!isfinite(d0)) { q.done = 1; q.status = 3; }
+        if (step == SC_INIT_MERGED && !q.done) q.restart = 1;  // merged iteration: the start is a restart of every active rhs (SC_RESTART2)
         break;
     case SC_ALPHA: {  // (d0,d1) = <r0, v>
         zs al = zero;
@@ -333,11 +396,74 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             q.r2 = q.maxr2 = d0;
             q.want_update = 0;
             if (!isfinite(d0)) { q.done = 1; q.status = 3; }
-            else if (d0 <= tol2 * q.eta2) { q.done = 1; q.beta = st_z(zero); }
+            else if (d0 <= tol2 * q.eta2) { q.done = 1; q.beta = q.gam = q.alpha = st_z(zero); }
         }
         break;
     case SC_RESTART:  // after r0 := r: rho = <r0, r> = ||r||^2 (the value SC_RHO / SC_TRUE left in r2)
         if (q.restart) { q.rho = make_double2(q.r2, 0.); q.beta = st_z(zero); q.restart = 0; }
+        break;
+    // ---- merged iteration (solver.cu): alpha is known before Mhat p, rho' comes from <r0,s> - omega <r0,t> ----
+    case SC_OMEGA2: {  // (d0,d1) = <t,s>, d2 = <t,t>, (e0,e1) = <r0,t>, (e2,e3) = <r0,s>
+        zs om = zero, be = zero, ga = zero;
+        q.want_update = 0;
+        q.claim = 0;
+        if (q.restart == 2) q.restart = 1;  // the minimal-residual step after a breakdown is done: restart before the next iteration
+        if (!q.done) {
+            if (!isfinite(d2) || !isfinite(d0) || !isfinite(d1) || !isfinite(e0) || !isfinite(e1) || !isfinite(e2) || !isfinite(e3)) {
+                q.done = 1; q.status = 3; q.alpha = st_z(zero);
+            } else {
+                if (d2 > 0.) om = zs{d0 / d2, d1 / d2};
+                const zs rho = ld_z(q.rho), rho1{e2 - (om.re * e0 - om.im * e1), e3 - (om.re * e1 + om.im * e0)};
+                const double om2 = om.re * om.re + om.im * om.im, rh2 = rho.re * rho.re + rho.im * rho.im;
+                if (!(om2 > 0.) || !(rh2 > 0.)) q.want_update = 1;  // stagnation: let the fp64 residual decide, beta = 0 gives p = r
+                else {
+                    ga = zdiv(rho1, rho);
+                    be = zmul(ga, zdiv(ld_z(q.alpha), om));
+                }
+                if (!finite_z(be) || !finite_z(ga) || q.restart) be = ga = zero;
+                q.rho = st_z(rho1);
+            }
+        }
+        q.omega = st_z(om);
+        q.beta = st_z(be);
+        q.gam = st_z(ga);
+        break;
+    }
+    case SC_RHO2: {  // (d0,d1) = <q0, p_new> = <r0, Mhat p_new>, d2 = ||r||^2
+        zs al = zero;
+        if (!q.done) {
+            q.r2 = d2;
+            if (d2 > q.maxr2) q.maxr2 = d2;
+            if (!isfinite(d2) || !isfinite(d0) || !isfinite(d1)) { q.done = 1; q.status = 3; }
+            else {
+                if (d2 < delta2 * q.maxr2) q.want_update = 1;
+                q.claim = (d2 <= tol2 * q.eta2) ? 1 : 0;
+                if (q.restart != 1) {  // (a restart recomputes alpha itself)
+                    if (d0 * d0 + d1 * d1 > 0.) al = zdiv(ld_z(q.rho), zs{d0, d1});
+                    if (!(d0 * d0 + d1 * d1 > 0.) || !finite_z(al)) {
+                        // breakdown: the next iteration is a pure minimal-residual step (alpha = 0), then r0 := r (R11)
+                        al = zero;
+                        if (q.nrestart < 8) { q.restart = 2; q.nrestart++; }
+                        else { q.done = 1; q.status = 2; }
+                    }
+                }
+            }
+        }
+        q.alpha = st_z(al);
+        break;
+    }
+    case SC_RESTART2:  // after r0 := p := r, q0 := Mhat^+ r0 for the flagged rhs: (d0,d1) = <q0, p>; rho = ||r||^2 (left in r2)
+        if (q.restart == 1) {
+            zs al = zero;
+            q.restart = 0;
+            q.rho = make_double2(q.r2, 0.);
+            q.beta = q.gam = st_z(zero);
+            if (!q.done) {
+                if (d0 * d0 + d1 * d1 > 0.) al = zdiv(ld_z(q.rho), zs{d0, d1});
+                if (!(d0 * d0 + d1 * d1 > 0.) || !finite_z(al)) { al = zero; q.done = 1; q.status = isfinite(d0) && isfinite(d1) ? 2 : 3; }
+            }
+            q.alpha = st_z(al);
+        }
         break;
     case SC_FINAL:  // d0 + d1 = ||eta - D psi||^2 on the full lattice; stored in r2 (true_r2 keeps the even-odd value)
         q.r2 = d0 + d1;
@@ -376,11 +502,41 @@ template <typename R> int blas_p_update(const BlasCtx &c, typename Vec<R>::T *p,
     CLV_CUDA(cudaGetLastError());
     return 0;
 }
-template <typename R> int blas_restart(const BlasCtx &c, const typename Vec<R>::T *r, typename Vec<R>::T *r0)
+template <typename R> int blas_restart(const BlasCtx &c, const typename Vec<R>::T *r, typename Vec<R>::T *r0, typename Vec<R>::T *p)
 {
     const size_t n = field_vecs<R>(*c.g, c.B);
-    restart_kernel<<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, r, r0);
+    restart_kernel<<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, r, r0, p);
     BLAS_LAUNCHED(c);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R>
+int blas_xrp_update(const BlasCtx &c, typename Vec<R>::T *x, typename Vec<R>::T *r, typename Vec<R>::T *p, const typename Vec<R>::T *s,
+                    const typename Vec<R>::T *t, const typename Vec<R>::T *q0, int *nblocks)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    const int grid = blas_grid(n);
+    xrp_update_kernel<<<grid, BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, x, r, p, s, t, q0, c.partial);
+    BLAS_LAUNCHED(c);
+    *nblocks = grid;
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R> int blas_gamma5(const BlasCtx &c, const typename Vec<R>::T *in, typename Vec<R>::T *out, int masked)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    gamma5_kernel<typename Vec<R>::T, Vec<R>::NV><<<blas_grid(n), BLAS_BLOCK, 0, c.st>>>(n, c.B, c.sc, masked, in, out);
+    BLAS_LAUNCHED(c);
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+template <typename R> int blas_cdot(const BlasCtx &c, const typename Vec<R>::T *a, const typename Vec<R>::T *b, int *nblocks)
+{
+    const size_t n = field_vecs<R>(*c.g, c.B);
+    const int grid = blas_grid(n);
+    cdot_kernel<<<grid, BLAS_BLOCK, 0, c.st>>>(n, c.B, a, b, c.partial);
+    BLAS_LAUNCHED(c);
+    *nblocks = grid;
     CLV_CUDA(cudaGetLastError());
     return 0;
 }
@@ -414,7 +570,8 @@ int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, cons
 }
 int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2)
 {
-    scalar_kernel<<<dim3(c.B, SC_SLICES), 256, 0, c.st>>>(step, c.B, nblocks, c.partial, c.sc, tol2, delta2, c.stage, c.ticket);
+    scalar_kernel<<<dim3(c.B, SC_SLICES), 256, 0, c.st>>>(step, c.B, nblocks, c.partial, step == SC_OMEGA2 ? c.partial2 : nullptr, c.sc, tol2, delta2, c.stage,
+                                                          c.ticket);
     BLAS_LAUNCHED(c);
     CLV_CUDA(cudaGetLastError());
     return 0;
@@ -425,7 +582,11 @@ int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, doubl
     template int blas_xr_update<R>(const BlasCtx &, Vec<R>::T *, Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *,          \
                                    const Vec<R>::T *, int *);                                                                                    \
     template int blas_p_update<R>(const BlasCtx &, Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *);                                           \
-    template int blas_restart<R>(const BlasCtx &, const Vec<R>::T *, Vec<R>::T *);                                                                \
+    template int blas_restart<R>(const BlasCtx &, const Vec<R>::T *, Vec<R>::T *, Vec<R>::T *);                                                                \
+    template int blas_xrp_update<R>(const BlasCtx &, Vec<R>::T *, Vec<R>::T *, Vec<R>::T *, const Vec<R>::T *, const Vec<R>::T *,                   \
+                                    const Vec<R>::T *, int *);                                                                                   \
+    template int blas_gamma5<R>(const BlasCtx &, const Vec<R>::T *, Vec<R>::T *, int);                                                           \
+    template int blas_cdot<R>(const BlasCtx &, const Vec<R>::T *, const Vec<R>::T *, int *);                                                     \
     template int blas_accumulate_y<R>(const BlasCtx &, double2 *, Vec<R>::T *);                                                                  \
     template int blas_residual<R>(const BlasCtx &, const double2 *, const double2 *, double2 *, Vec<R>::T *, int *);
 INST(float)

@@ -12,8 +12,9 @@ struct BlasCtx {
     int B;
     RhsScalars *sc;    // device, B entries
     double *partial;   // device, [blocks][B][4]
+    double *partial2;  // device, same shape: second plane of the DOT_XW epilogue (merged iteration)
     int max_partial_blocks;
-    double *stage;     // device, [8 rhs][32 slices][4]: second-level partials of the scalar kernels
+    double *stage;     // device, [8 rhs][32 slices][8]: second-level partials of the scalar kernels
     unsigned *ticket;  // device, [8]: arrival counters of the scalar kernels (zero between launches)
     cudaStream_t st;
     long long *launches;
@@ -35,9 +36,18 @@ template <typename R> int blas_residual(const BlasCtx &c, const double2 *b, cons
 int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, const double2 *a2, const double2 *b2, int *nblocks);
 
 // scalar steps (one block per rhs): reduce the partials of `nblocks` blocks and update RhsScalars
-enum { SC_ETA2 = 0, SC_INIT = 1, SC_ALPHA = 2, SC_OMEGA = 3, SC_RHO = 4, SC_TRUE = 5, SC_FINAL = 6, SC_RESTART = 7 };
+enum { SC_ETA2 = 0, SC_INIT = 1, SC_ALPHA = 2, SC_OMEGA = 3, SC_RHO = 4, SC_TRUE = 5, SC_FINAL = 6, SC_RESTART = 7,
+       SC_INIT_MERGED = 8, SC_OMEGA2 = 9, SC_RHO2 = 10, SC_RESTART2 = 11 };  // merged iteration (solver.cu)
 // r0 = r for the rhs whose `restart` flag is set (breakdown recovery)
-template <typename R> int blas_restart(const BlasCtx &c, const typename Vec<R>::T *r, typename Vec<R>::T *r0);
+template <typename R> int blas_restart(const BlasCtx &c, const typename Vec<R>::T *r, typename Vec<R>::T *r0, typename Vec<R>::T *p = nullptr);
+// merged iteration: x += alpha p + omega s ; r' = s - omega t ; p = r' + beta p - gam (r - s) ; partial <q0,p>, ||r'||^2
+template <typename R>
+int blas_xrp_update(const BlasCtx &c, typename Vec<R>::T *x, typename Vec<R>::T *r, typename Vec<R>::T *p, const typename Vec<R>::T *s,
+                    const typename Vec<R>::T *t, const typename Vec<R>::T *q0, int *nblocks);
+// out = gamma5 in (masked: only the rhs flagged restart == 1 are written)
+template <typename R> int blas_gamma5(const BlasCtx &c, const typename Vec<R>::T *in, typename Vec<R>::T *out, int masked);
+// partial <a, b>
+template <typename R> int blas_cdot(const BlasCtx &c, const typename Vec<R>::T *a, const typename Vec<R>::T *b, int *nblocks);
 int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2);
 
 }  // namespace clv

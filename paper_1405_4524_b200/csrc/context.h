@@ -18,6 +18,7 @@ template <typename R> struct OpData {
 // Per-rhs solver scalars, device resident (one entry per rhs of the batch).
 struct RhsScalars {
     double2 rho, alpha, omega, beta;  // BiCGStab recurrences (complex)
+    double2 gam;      // merged iteration: rho'/rho = beta omega / alpha, the coefficient of (r - s) = alpha v in the p update
     double r2;        // ||r||^2 of the iterated (sloppy) residual
     double maxr2;     // max ||r||^2 since the last reliable update
     double eta2;      // ||eta||^2 on the full lattice (stopping scale, R10)
@@ -60,7 +61,9 @@ int reorder_out(const Geom &g, CT *canon, const typename Vec<R>::T *even, const 
 // ---- dslash.cu ----
 // out = P ( X + coef * H_{p,1-p} in ),  P = 1 | A_pp^-1,  X = 0 | xin | A_pp xin   (p = parity of out)
 enum { XM_NONE = 0, XM_PLAIN = 1, XM_CLOVER = 2 };
-enum { DOT_NONE = 0, DOT_W = 1, DOT_X = 2, DOT_RES = 3 };
+// DOT_S / DOT_XW are the epilogues of the merged BiCGStab iteration (solver.cu): DOT_S computes v = (...) but stores only s = w - alpha v
+// (to `out2`; `out` is not written) (alpha = sc[rhs].alpha, already known when the kernel starts; no reduction); DOT_XW is DOT_X plus <w, out> and <w, xin>.
+enum { DOT_NONE = 0, DOT_W = 1, DOT_X = 2, DOT_RES = 3, DOT_S = 4, DOT_XW = 5 };
 template <typename R> struct DslashArgs {
     typedef typename Vec<R>::T V;
     const V *in;      // parity 1-p field
@@ -69,6 +72,9 @@ template <typename R> struct DslashArgs {
     const V *w;       // DOT_W: partial <w, out> per rhs.  DOT_RES: the result is w - (...), partial ||result||^2
     float4 *out32;    // DOT_RES only: if non-null the result is stored here in fp32 instead of `out` (reliable update: r = b - Mhat y)
     double *partial;  // [gridDim.x][B][4] : DOT_W -> (re,im of <w,out>, 0, 0); DOT_X -> (re,im of <out,xin>, <out,out>, 0)
+    double *partial2; // DOT_XW: second plane, same shape: (re,im of <w,out>, re,im of <w,xin>)
+    V *out2;          // DOT_S: s = w - alpha * result (the only store of that variant)
+    const RhsScalars *sc;  // DOT_S: per-rhs scalars (alpha)
     R coef;
     int parity;       // p
     int xmode, pinv, dot;

@@ -180,14 +180,16 @@ __device__ __forceinline__ void clover_mul2(const float2 *__restrict__ clov, uns
     }
 }
 
-// per-rhs block reduction when a thread holds the partial sums of rhs 2q and 2q+1, q = threadIdx.x % (B/2)
-template <int B, int BLOCK> __device__ __forceinline__ void block_reduce_pair(double vA[3], double vB[3], double *__restrict__ partial)
+// per-rhs block reduction when a thread holds the partial sums of rhs 2q and 2q+1, q = threadIdx.x % (B/2); N = 3 sums per rhs
+// into `partial`, or N = 7 (DOT_XW): sums 0..2 into `partial`, 3..6 into slots 0..3 of `partial2`
+template <int B, int BLOCK, int N>
+__device__ __forceinline__ void block_reduce_pair(double vA[N], double vB[N], double *__restrict__ partial, double *__restrict__ partial2)
 {
-    __shared__ double sm[BLOCK / 32][B][3];
+    __shared__ double sm[BLOCK / 32][B][N];
 #pragma unroll
     for (int off = 16; off >= B / 2 && off >= 1; off >>= 1) {
 #pragma unroll
-        for (int c = 0; c < 3; c++) {
+        for (int c = 0; c < N; c++) {
             vA[c] += __shfl_xor_sync(0xffffffffu, vA[c], off);
             vB[c] += __shfl_xor_sync(0xffffffffu, vB[c], off);
         }
@@ -195,38 +197,62 @@ template <int B, int BLOCK> __device__ __forceinline__ void block_reduce_pair(do
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (lane < B / 2) {
 #pragma unroll
-        for (int c = 0; c < 3; c++) {
+        for (int c = 0; c < N; c++) {
             sm[warp][2 * lane][c] = vA[c];
             sm[warp][2 * lane + 1][c] = vB[c];
         }
     }
     __syncthreads();
-    if (threadIdx.x < B * 3) {
-        const int r = threadIdx.x / 3, c = threadIdx.x % 3;
+    if (threadIdx.x < B * N) {
+        const int r = threadIdx.x / N, c = threadIdx.x % N;
         double s = 0;
 #pragma unroll
         for (int w = 0; w < BLOCK / 32; w++) s += sm[w][r][c];
-        partial[((size_t)blockIdx.x * B + r) * 4 + c] = s;
+        if (c < 3) partial[((size_t)blockIdx.x * B + r) * 4 + c] = s;
+        else partial2[((size_t)blockIdx.x * B + r) * 4 + (c - 3)] = s;
     }
 }
 
-// epilogue dot products of one rhs (same definitions as dslash_kernel)
-template <int DOT> __device__ __forceinline__ void dots(const cx<float> acc[12], const cx<float> x[12], const cx<float> w[12], double d[3])
+// epilogue dot products of one rhs (same definitions as dslash_kernel).  The 12 terms of a site are summed in fp32 and converted
+// once: the fp64 pipe and the F2F converter are slow enough that 12 conversions + 12 DADD per sum showed up in the kernel time
+// (DOT_XW has seven sums); the accumulation across sites stays fp64.
+template <int DOT> __device__ __forceinline__ void dots(const cx<float> acc[12], const cx<float> x[12], const cx<float> w[12], double *d)
 {
     if (DOT == DOT_W) {
+        float f0 = 0.f, f1 = 0.f;
 #pragma unroll
         for (int i = 0; i < 12; i++) {  // <w, out>
-            d[0] += (double)(w[i].re * acc[i].re + w[i].im * acc[i].im);
-            d[1] += (double)(w[i].re * acc[i].im - w[i].im * acc[i].re);
+            f0 += w[i].re * acc[i].re + w[i].im * acc[i].im;
+            f1 += w[i].re * acc[i].im - w[i].im * acc[i].re;
         }
+        d[0] += (double)f0;
+        d[1] += (double)f1;
     }
-    if (DOT == DOT_X) {
+    if (DOT == DOT_X || DOT == DOT_XW) {
+        float f0 = 0.f, f1 = 0.f, f2 = 0.f;
 #pragma unroll
         for (int i = 0; i < 12; i++) {  // <out, xin>, <out, out>
-            d[0] += (double)(acc[i].re * x[i].re + acc[i].im * x[i].im);
-            d[1] += (double)(acc[i].re * x[i].im - acc[i].im * x[i].re);
-            d[2] += (double)(acc[i].re * acc[i].re + acc[i].im * acc[i].im);
+            f0 += acc[i].re * x[i].re + acc[i].im * x[i].im;
+            f1 += acc[i].re * x[i].im - acc[i].im * x[i].re;
+            f2 += acc[i].re * acc[i].re + acc[i].im * acc[i].im;
         }
+        d[0] += (double)f0;
+        d[1] += (double)f1;
+        d[2] += (double)f2;
+    }
+    if (DOT == DOT_XW) {
+        float f3 = 0.f, f4 = 0.f, f5 = 0.f, f6 = 0.f;
+#pragma unroll
+        for (int i = 0; i < 12; i++) {  // <w, out>, <w, xin>
+            f3 += w[i].re * acc[i].re + w[i].im * acc[i].im;
+            f4 += w[i].re * acc[i].im - w[i].im * acc[i].re;
+            f5 += w[i].re * x[i].re + w[i].im * x[i].im;
+            f6 += w[i].re * x[i].im - w[i].im * x[i].re;
+        }
+        d[3] += (double)f3;
+        d[4] += (double)f4;
+        d[5] += (double)f5;
+        d[6] += (double)f6;
     }
 }
 
@@ -240,7 +266,8 @@ dslash2_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
     static_assert(B >= 2 && B % 2 == 0, "pairs of right-hand sides");
     const unsigned j = 2u * (blockIdx.x * BLOCK + threadIdx.x);   // first rhs of this thread's pair
     const bool active = j < (unsigned)g.Vh * B;
-    double dA[3] = {0, 0, 0}, dB[3] = {0, 0, 0};
+    constexpr int ND = DOT == DOT_XW ? 7 : 3;
+    double dA[ND] = {}, dB[ND] = {};
     const int p = a.parity;
     constexpr int SITES = 2 * BLOCK / B;   // sites of this CTA: consecutive cb from blockIdx.x * SITES
     __shared__ __align__(16) float4 cl_s[(CLV_R2_SMEM && (XMODE == XM_CLOVER || PINV)) ? SITES * 18 : 1];
@@ -307,7 +334,7 @@ dslash2_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
             }
         }
         cx<float> wA[12], wB[12];
-        if (DOT == DOT_W || DOT == DOT_RES) load_spinor2(a.w, j, wA, wB);
+        if (DOT == DOT_W || DOT == DOT_RES || DOT == DOT_S || DOT == DOT_XW) load_spinor2(a.w, j, wA, wB);
         if (DOT == DOT_RES) {  // result = w - acc, ||result||^2 (fp32 iteration precision: out32 and out are the same type here)
 #pragma unroll
             for (int i = 0; i < 12; i++) {
@@ -317,11 +344,22 @@ dslash2_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
                 dB[0] += (double)accB[i].re * (double)accB[i].re + (double)accB[i].im * (double)accB[i].im;
             }
         }
-        store_spinor2((DOT == DOT_RES && a.out32) ? a.out32 : a.out, j, accA, accB);
+        if (DOT != DOT_S) store_spinor2((DOT == DOT_RES && a.out32) ? a.out32 : a.out, j, accA, accB);
+        if (DOT == DOT_S) {  // merged iteration: v stays in registers, out2 = s = w - alpha v with w = r
+            const int rhs = j % B;
+            const double2 alA = a.sc[rhs].alpha, alB = a.sc[rhs + 1].alpha;
+            const cx<float> mA = mk<float>((float)-alA.x, (float)-alA.y), mB = mk<float>((float)-alB.x, (float)-alB.y);
+#pragma unroll
+            for (int i = 0; i < 12; i++) {
+                fma_cx(wA[i], mA, accA[i]);
+                fma_cx(wB[i], mB, accB[i]);
+            }
+            store_spinor2(a.out2, j, wA, wB);
+        }
         dots<DOT>(accA, xA, wA, dA);
         dots<DOT>(accB, xB, wB, dB);
     }
-    if (DOT != DOT_NONE) block_reduce_pair<B, BLOCK>(dA, dB, a.partial);
+    if (DOT != DOT_NONE && DOT != DOT_S) block_reduce_pair<B, BLOCK, ND>(dA, dB, a.partial, a.partial2);
 }
 
 }  // namespace clv

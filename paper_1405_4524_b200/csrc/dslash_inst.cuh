@@ -6,19 +6,22 @@
 
 namespace clv {
 
+// variants with a per-CTA reduction keep DSLASH_BLOCK threads; the others (DOT_NONE, DOT_S) run one-warp CTAs
+#define CLV_HAS_RED(DT) ((DT) != DOT_NONE && (DT) != DOT_S)
+
 // fp32, B >= 2: the (site, rhs-pair) kernel of dslash2_kernel.cuh
 template <int B, int RECON>
 static int launch_dslash2_BR(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
 {
     const Geom &g = ctx->geom;
     const unsigned npairs = (unsigned)g.Vh * B / 2;
-    const unsigned block = a.dot == DOT_NONE ? CLV_R2_BLOCK_NODOT : DSLASH_BLOCK;
+    const unsigned block = CLV_HAS_RED(a.dot) ? DSLASH_BLOCK : CLV_R2_BLOCK_NODOT;
     const unsigned grid = (npairs + block - 1) / block;
     if (grid_out) *grid_out = (int)grid;
     const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
 #define CLV_LAUNCH2(XM, PI, DT)                                                      \
     case (XM) * 100 + (PI) * 10 + (DT):                                              \
-        dslash2_kernel<B, RECON, XM, PI, DT, ((DT) == DOT_NONE ? CLV_R2_BLOCK_NODOT : DSLASH_BLOCK)><<<grid, block, 0, st>>>(g, op, a); \
+        dslash2_kernel<B, RECON, XM, PI, DT, (CLV_HAS_RED(DT) ? DSLASH_BLOCK : CLV_R2_BLOCK_NODOT)><<<grid, block, 0, st>>>(g, op, a); \
         break;
     switch (key) {
         CLV_LAUNCH2(XM_NONE, 0, DOT_NONE)
@@ -29,6 +32,8 @@ static int launch_dslash2_BR(const clover_ctx *ctx, const OpData<float> &op, con
         CLV_LAUNCH2(XM_CLOVER, 0, DOT_W)
         CLV_LAUNCH2(XM_CLOVER, 0, DOT_X)
         CLV_LAUNCH2(XM_CLOVER, 0, DOT_RES)
+        CLV_LAUNCH2(XM_CLOVER, 0, DOT_S)
+        CLV_LAUNCH2(XM_CLOVER, 0, DOT_XW)
     default:
         set_error("dslash: unsupported variant xmode=%d pinv=%d dot=%d", a.xmode, a.pinv, a.dot);
         return CLOVER_EINVAL;
@@ -64,13 +69,13 @@ static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const Ds
     if (PairLaunch<R, B, RECON>::use() && (a.xmode != XM_NONE || a.pinv)) return PairLaunch<R, B, RECON>::go(ctx, op, a, st, grid_out);
     const Geom &g = ctx->geom;
     const unsigned n = (unsigned)g.Vh * B;
-    const unsigned block = a.dot == DOT_NONE ? CLV_DSLASH_BLOCK_NODOT : DSLASH_BLOCK;
+    const unsigned block = CLV_HAS_RED(a.dot) ? DSLASH_BLOCK : CLV_DSLASH_BLOCK_NODOT;
     const unsigned grid = (n + block - 1) / block;
     if (grid_out) *grid_out = (int)grid;
     const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
 #define CLV_LAUNCH(XM, PI, DT)                                                          \
     case (XM) * 100 + (PI) * 10 + (DT):                                                 \
-        dslash_kernel<R, B, RECON, XM, PI, DT, ((DT) == DOT_NONE ? CLV_DSLASH_BLOCK_NODOT : DSLASH_BLOCK)><<<grid, block, 0, st>>>(g, op, a); \
+        dslash_kernel<R, B, RECON, XM, PI, DT, (CLV_HAS_RED(DT) ? DSLASH_BLOCK : CLV_DSLASH_BLOCK_NODOT)><<<grid, block, 0, st>>>(g, op, a); \
         break;
     switch (key) {
         CLV_LAUNCH(XM_NONE, 0, DOT_NONE)
@@ -81,6 +86,8 @@ static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const Ds
         CLV_LAUNCH(XM_CLOVER, 0, DOT_W)
         CLV_LAUNCH(XM_CLOVER, 0, DOT_X)
         CLV_LAUNCH(XM_CLOVER, 0, DOT_RES)
+        CLV_LAUNCH(XM_CLOVER, 0, DOT_S)
+        CLV_LAUNCH(XM_CLOVER, 0, DOT_XW)
     default:
         set_error("dslash: unsupported variant xmode=%d pinv=%d dot=%d", a.xmode, a.pinv, a.dot);
         return CLOVER_EINVAL;

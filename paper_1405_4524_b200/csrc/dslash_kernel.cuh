@@ -296,6 +296,31 @@ template <int B, int BLOCK> __device__ __forceinline__ void block_reduce_rhs(dou
     }
 }
 
+// DOT_XW: seven sums per rhs; v[0..2] go to plane `partial` (slots 0..2), v[3..6] to plane `partial2` (slots 0..3)
+template <int B, int BLOCK> __device__ __forceinline__ void block_reduce_rhs7(double v[7], double *__restrict__ partial, double *__restrict__ partial2)
+{
+    __shared__ double sm[BLOCK / 32][B][7];
+#pragma unroll
+    for (int off = 16; off >= B; off >>= 1) {
+#pragma unroll
+        for (int c = 0; c < 7; c++) v[c] += __shfl_xor_sync(0xffffffffu, v[c], off);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane < B) {
+#pragma unroll
+        for (int c = 0; c < 7; c++) sm[warp][lane][c] = v[c];
+    }
+    __syncthreads();
+    if (threadIdx.x < B * 7) {
+        const int r = threadIdx.x / 7, c = threadIdx.x % 7;
+        double s = 0;
+#pragma unroll
+        for (int w = 0; w < BLOCK / 32; w++) s += sm[w][r][c];
+        if (c < 3) partial[((size_t)blockIdx.x * B + r) * 4 + c] = s;
+        else partial2[((size_t)blockIdx.x * B + r) * 4 + (c - 3)] = s;
+    }
+}
+
 // L1 prefetch of everything the epilogue will read (clover blocks, xin, w): issued part-way through the hop so that the
 // epilogue's loads -- first touches of DRAM lines, at the end of a dependent chain -- do not stall the warp for a full
 // DRAM round trip with no registers left to overlap it.
@@ -315,7 +340,7 @@ __device__ __forceinline__ void prefetch_epilogue(const OpData<R> &op, const Dsl
 #pragma unroll
         for (int k = 0; k < NV; k++) prefetch_l1(q + 32 * k);
     }
-    if (DOT == DOT_W || DOT == DOT_RES) {
+    if (DOT == DOT_W || DOT == DOT_RES || DOT == DOT_S || DOT == DOT_XW) {
         const typename Vec<R>::T *q = a.w + lb_index(j, 0, NV);
 #pragma unroll
         for (int k = 0; k < NV; k++) prefetch_l1(q + 32 * k);
@@ -344,7 +369,7 @@ __global__ void __launch_bounds__(BLOCK, (sizeof(R) == 8 ? CLV_DSLASH_MINB64 : C
 {
     const unsigned j = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = j < (unsigned)g.Vh * B;
-    double d0 = 0, d1 = 0, d2 = 0;
+    double d0 = 0, d1 = 0, d2 = 0, d3 = 0, d4 = 0, d5 = 0, d6 = 0;
     if (active) {
         const int cb = j / B, rhs = j % B, p = a.parity;
         const Coord c = decode(g, cb, p);
@@ -409,26 +434,60 @@ __global__ void __launch_bounds__(BLOCK, (sizeof(R) == 8 ? CLV_DSLASH_MINB64 : C
                 for (int i = 0; i < 12; i++) f[i] = mk<float>((float)acc[i].re, (float)acc[i].im);
                 store_spinor(a.out32, j, f);
             } else if (a.out) store_spinor(a.out, j, acc);   // neither: only the norm is wanted (final verification)
-        } else store_spinor(a.out, j, acc);
+        } else if (DOT != DOT_S) store_spinor(a.out, j, acc);
+        if (DOT == DOT_S) {  // merged iteration: v stays in registers, out2 = s = w - alpha v with w = r
+            cx<R> w[12];
+            load_spinor(a.w, j, w);
+            const double2 al = a.sc[rhs].alpha;
+            const cx<R> mal = mk<R>((R)-al.x, (R)-al.y);
+#pragma unroll
+            for (int i = 0; i < 12; i++) fma_cx(w[i], mal, acc[i]);
+            store_spinor(a.out2, j, w);
+        }
+        // dot products: the 12 terms of a site are summed in the kernel's precision and converted once (fp32: the F2F converter
+        // and the fp64 pipe are slow); the accumulation across sites is fp64
+        if (DOT == DOT_XW) {  // merged iteration: <out,xin>, <out,out>, <w,out>, <w,xin> with out = t, xin = s, w = r0
+            cx<R> w[12];
+            load_spinor(a.w, j, w);
+            R f0 = 0, f1 = 0, f2 = 0, f3 = 0, f4 = 0, f5 = 0, f6 = 0;
+#pragma unroll
+            for (int i = 0; i < 12; i++) {
+                f0 += acc[i].re * x[i].re + acc[i].im * x[i].im;
+                f1 += acc[i].re * x[i].im - acc[i].im * x[i].re;
+                f2 += acc[i].re * acc[i].re + acc[i].im * acc[i].im;
+                f3 += w[i].re * acc[i].re + w[i].im * acc[i].im;
+                f4 += w[i].re * acc[i].im - w[i].im * acc[i].re;
+                f5 += w[i].re * x[i].re + w[i].im * x[i].im;
+                f6 += w[i].re * x[i].im - w[i].im * x[i].re;
+            }
+            d0 = (double)f0; d1 = (double)f1; d2 = (double)f2; d3 = (double)f3; d4 = (double)f4; d5 = (double)f5; d6 = (double)f6;
+        }
         if (DOT == DOT_W) {
             cx<R> w[12];
             load_spinor(a.w, j, w);
+            R f0 = 0, f1 = 0;
 #pragma unroll
             for (int i = 0; i < 12; i++) {  // <w, out> = sum conj(w) out
-                d0 += (double)(w[i].re * acc[i].re + w[i].im * acc[i].im);
-                d1 += (double)(w[i].re * acc[i].im - w[i].im * acc[i].re);
+                f0 += w[i].re * acc[i].re + w[i].im * acc[i].im;
+                f1 += w[i].re * acc[i].im - w[i].im * acc[i].re;
             }
+            d0 = (double)f0; d1 = (double)f1;
         }
         if (DOT == DOT_X) {
+            R f0 = 0, f1 = 0, f2 = 0;
 #pragma unroll
             for (int i = 0; i < 12; i++) {  // <out, xin> and <out, out>
-                d0 += (double)(acc[i].re * x[i].re + acc[i].im * x[i].im);
-                d1 += (double)(acc[i].re * x[i].im - acc[i].im * x[i].re);
-                d2 += (double)(acc[i].re * acc[i].re + acc[i].im * acc[i].im);
+                f0 += acc[i].re * x[i].re + acc[i].im * x[i].im;
+                f1 += acc[i].re * x[i].im - acc[i].im * x[i].re;
+                f2 += acc[i].re * acc[i].re + acc[i].im * acc[i].im;
             }
+            d0 = (double)f0; d1 = (double)f1; d2 = (double)f2;
         }
     }
-    if (DOT != DOT_NONE) block_reduce_rhs<B, BLOCK>(d0, d1, d2, a.partial);
+    if (DOT == DOT_XW) {
+        double d[7] = {d0, d1, d2, d3, d4, d5, d6};
+        block_reduce_rhs7<B, BLOCK>(d, a.partial, a.partial2);
+    } else if (DOT != DOT_NONE && DOT != DOT_S) block_reduce_rhs<B, BLOCK>(d0, d1, d2, a.partial);
 }
 
 // standalone clover apply: out = A in or A^-1 in

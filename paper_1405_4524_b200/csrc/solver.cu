@@ -16,8 +16,8 @@ struct SolveWork {
     int B_cap = 0;
     size_t sloppy_bytes = 0;   // bytes of each sloppy field currently allocated
     double2 *f64[8] = {};      // eta_e, eta_o, b, y, r64, w64, tmp64, psi_o
-    void *sl[8] = {};          // x, r, p, v, s, t, r0, tmp  (float4 or double2 fields)
-    double *partial = nullptr;
+    void *sl[9] = {};          // x, r, p, v, s, t, r0, tmp, q0  (float4 or double2 fields)
+    double *partial = nullptr, *partial2 = nullptr;
     int partial_blocks = 0;
     double *stage = nullptr;
     unsigned *ticket = nullptr;
@@ -37,19 +37,21 @@ struct SolveWork {
     cudaStream_t s_work = nullptr;
     cudaEvent_t ev_dep = nullptr;
     cudaGraphExec_t iter_graph = nullptr;
-    int graph_B = 0, graph_prec = 0, graph_kernels = 0;
+    int graph_B = 0, graph_prec = 0, graph_kernels = 0, graph_merged = -1;
     double graph_tol2 = 0, graph_delta2 = 0;
 };
 
 enum { F_ETA_E = 0, F_ETA_O, F_B, F_Y, F_R64, F_W64, F_TMP64, F_PSI_O };
-enum { S_X = 0, S_R, S_P, S_V, S_S, S_T, S_R0, S_TMP };
+enum { S_X = 0, S_R, S_P, S_V, S_S, S_T, S_R0, S_TMP, S_Q0, S_NFIELDS };
 
 void free_work(clover_ctx *ctx)
 {
     SolveWork *W = ctx->work;
     if (!W) return;
-    for (int i = 0; i < 8; i++) { cudaFree(W->f64[i]); cudaFree(W->sl[i]); }
+    for (int i = 0; i < 8; i++) cudaFree(W->f64[i]);
+    for (int i = 0; i < S_NFIELDS; i++) cudaFree(W->sl[i]);
     cudaFree(W->partial);
+    cudaFree(W->partial2);
     cudaFree(W->stage);
     cudaFree(W->ticket);
     cudaFree(W->sc_dev);
@@ -84,12 +86,15 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
         W->partial_blocks = 2 * std::max<int>(((unsigned)g.Vh * B + dslash_block_size() - 1) / dslash_block_size(), 148 * 8);
         CLV_CUDA(cudaMalloc(&W->partial, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
         CLV_CUDA(cudaMemset(W->partial, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
+        cudaFree(W->partial2);
+        CLV_CUDA(cudaMalloc(&W->partial2, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
+        CLV_CUDA(cudaMemset(W->partial2, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
         if (!W->sc_dev) {
             CLV_CUDA(cudaMalloc(&W->sc_dev, 8 * sizeof(RhsScalars)));
             CLV_CUDA(cudaMemset(W->sc_dev, 0, 8 * sizeof(RhsScalars)));
             CLV_CUDA(cudaHostAlloc((void **)&W->sc_host, 8 * sizeof(RhsScalars), cudaHostAllocMapped));
             CLV_CUDA(cudaHostGetDevicePointer((void **)&W->sc_host_dev, W->sc_host, 0));
-            CLV_CUDA(cudaMalloc(&W->stage, 8 * 32 * 4 * sizeof(double)));
+            CLV_CUDA(cudaMalloc(&W->stage, 8 * 32 * 8 * sizeof(double)));
             CLV_CUDA(cudaMalloc(&W->ticket, 8 * sizeof(unsigned)));
             CLV_CUDA(cudaMemset(W->ticket, 0, 8 * sizeof(unsigned)));
         }
@@ -99,7 +104,7 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
     }
     const size_t need = field_vecs<double>(g, W->B_cap) * 16 / 8 * real_bytes;  // float fields are half the size of double ones
     if (need > W->sloppy_bytes) {
-        for (int i = 0; i < 8; i++) {
+        for (int i = 0; i < S_NFIELDS; i++) {
             cudaFree(W->sl[i]);
             W->sl[i] = nullptr;
             CLV_CUDA(cudaMalloc(&W->sl[i], need));
@@ -146,10 +151,8 @@ static int clear_fields(SolveWork *W, const Geom &g, int B, cudaStream_t st)
 {
     if (((unsigned)g.Vh * B) % 32u == 0) return 0;
     const size_t n64 = field_vecs<double>(g, W->B_cap) * sizeof(double2);
-    for (int i = 0; i < 8; i++) {
-        CLV_CUDA(cudaMemsetAsync(W->f64[i], 0, n64, st));
-        CLV_CUDA(cudaMemsetAsync(W->sl[i], 0, W->sloppy_bytes, st));
-    }
+    for (int i = 0; i < 8; i++) CLV_CUDA(cudaMemsetAsync(W->f64[i], 0, n64, st));
+    for (int i = 0; i < S_NFIELDS; i++) CLV_CUDA(cudaMemsetAsync(W->sl[i], 0, W->sloppy_bytes, st));
     return 0;
 }
 
@@ -158,6 +161,7 @@ template <typename R> static DslashArgs<R> dargs(const typename Vec<R>::T *in, c
 {
     DslashArgs<R> a;
     a.in = in; a.xin = xin; a.out = out; a.w = w; a.out32 = nullptr; a.partial = partial; a.coef = coef; a.parity = parity;
+    a.partial2 = nullptr; a.out2 = nullptr; a.sc = nullptr;
     a.xmode = xmode; a.pinv = pinv; a.dot = dot;
     return a;
 }
@@ -165,7 +169,8 @@ template <typename R> static DslashArgs<R> dargs(const typename Vec<R>::T *in, c
 // out_e = Mhat in_e, optional fused dot products; tmp is an odd-parity scratch field
 template <typename R>
 static int mhat(clover_ctx *ctx, int B, const typename Vec<R>::T *in, typename Vec<R>::T *tmp, typename Vec<R>::T *out, int dot, const typename Vec<R>::T *w,
-                double *partial, int *grid, cudaStream_t st, cudaEvent_t *kev = nullptr, float4 *out32 = nullptr)
+                double *partial, int *grid, cudaStream_t st, cudaEvent_t *kev = nullptr, float4 *out32 = nullptr, typename Vec<R>::T *out2 = nullptr,
+                double *partial2 = nullptr, const RhsScalars *sc = nullptr)
 {
     const R k2 = (R)(-ctx->kappa * ctx->kappa);
     if (kev) CLV_CUDA(cudaEventRecord(kev[0], st));
@@ -173,6 +178,9 @@ static int mhat(clover_ctx *ctx, int B, const typename Vec<R>::T *in, typename V
     if (kev) CLV_CUDA(cudaEventRecord(kev[1], st));
     DslashArgs<R> a2 = dargs<R>(tmp, in, out, k2, 0, XM_CLOVER, 0, dot, w, partial);
     a2.out32 = out32;
+    a2.out2 = out2;
+    a2.partial2 = partial2;
+    a2.sc = sc;
     CLV_CHECK(launch_dslash<R>(ctx, a2, B, st, grid));
     if (kev) CLV_CUDA(cudaEventRecord(kev[2], st));
     ctx->stats.kernel_launches += 2;
@@ -217,6 +225,16 @@ static bool graph_enabled(const Geom &g, int B)
     return (size_t)g.Vh * B * 96 < ((size_t)64 << 20);
 }
 
+// The merged iteration (default) moves BLAS-1 traffic into the Dslash epilogues: alpha is known before Mhat p is applied
+// (<r0, Mhat p> = <Mhat^+ r0, p>, Mhat^+ = gamma5 Mhat gamma5), so the second Dslash of Mhat p stores s = r - alpha v instead of v, the
+// second Dslash of Mhat s also returns <r0,t> and <r0,s> (rho' = <r0,s> - omega <r0,t>), and one sweep does the x, r and p updates
+// (p = r' + beta p - (rho'/rho)(r - s), since r - s = alpha v): 9 vector passes + 2 scalar steps per iteration instead of 14 + 3.  CLOVER_MERGED=0 selects the textbook ordering.
+static bool merged_enabled()
+{
+    const char *e = getenv("CLOVER_MERGED");  // tuning/debug knob only
+    return e ? atoi(e) != 0 : true;
+}
+
 template <typename R>
 static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, double tol, int max_iter, clover_rhs_info *info, cudaStream_t st_user)
 {
@@ -233,9 +251,10 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     double2 *eta_e = W->f64[F_ETA_E], *eta_o = W->f64[F_ETA_O], *b = W->f64[F_B], *y = W->f64[F_Y], *r64 = W->f64[F_R64],
             *tmp64 = W->f64[F_TMP64], *psi_o = W->f64[F_PSI_O];
     V *x = (V *)W->sl[S_X], *r = (V *)W->sl[S_R], *p = (V *)W->sl[S_P], *v = (V *)W->sl[S_V], *s = (V *)W->sl[S_S], *t = (V *)W->sl[S_T],
-      *r0 = (V *)W->sl[S_R0], *tmp = (V *)W->sl[S_TMP];
+      *r0 = (V *)W->sl[S_R0], *tmp = (V *)W->sl[S_TMP], *q0 = (V *)W->sl[S_Q0];
+    const bool merged = merged_enabled();
     long long &nl = ctx->stats.kernel_launches;
-    BlasCtx bc{&g, B, W->sc_dev, W->partial, W->partial_blocks, W->stage, W->ticket, st, &nl};
+    BlasCtx bc{&g, B, W->sc_dev, W->partial, W->partial2, W->partial_blocks, W->stage, W->ticket, st, &nl};
     const double tol2 = tol * tol, delta = reliable_delta(), delta2 = delta * delta;
     const size_t nbytes = field_vecs<R>(g, B) * sizeof(V), nbytes64 = field_vecs<double>(g, B) * sizeof(double2);
     int nb = 0, grid = 0, iters = 0, updates = 0;
@@ -255,9 +274,23 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     CLV_CUDA(cudaMemsetAsync(y, 0, nbytes64, st));
     CLV_CUDA(cudaMemsetAsync(x, 0, nbytes, st));
     CLV_CHECK(blas_residual<R>(bc, b, nullptr, r64, r, &nb));
-    CLV_CHECK(blas_scalar_step(bc, SC_INIT, nb, tol2, delta2));
-    CLV_CUDA(cudaMemcpyAsync(p, r, nbytes, cudaMemcpyDeviceToDevice, st));
-    CLV_CUDA(cudaMemcpyAsync(r0, r, nbytes, cudaMemcpyDeviceToDevice, st));
+    CLV_CHECK(blas_scalar_step(bc, merged ? SC_INIT_MERGED : SC_INIT, nb, tol2, delta2));
+    // merged iteration, (re)start of the rhs flagged `restart == 1`: r0 := p := r, q0 := Mhat^+ r0 = gamma5 Mhat gamma5 r0,
+    // rho := ||r||^2, alpha := rho / <q0, p>.  s, t and tmp are free between iterations and serve as scratch.
+    auto restart_merged = [&]() -> int {
+        CLV_CHECK(blas_restart<R>(bc, r, r0, p));
+        CLV_CHECK(blas_gamma5<R>(bc, r0, s, 0));
+        CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_NONE, nullptr, nullptr, nullptr, st));
+        CLV_CHECK(blas_gamma5<R>(bc, t, q0, 1));
+        CLV_CHECK(blas_cdot<R>(bc, q0, p, &nb));
+        CLV_CHECK(blas_scalar_step(bc, SC_RESTART2, nb, tol2, delta2));
+        return 0;
+    };
+    if (merged) CLV_CHECK(restart_merged());
+    else {
+        CLV_CUDA(cudaMemcpyAsync(p, r, nbytes, cudaMemcpyDeviceToDevice, st));
+        CLV_CUDA(cudaMemcpyAsync(r0, r, nbytes, cudaMemcpyDeviceToDevice, st));
+    }
     CLV_CUDA(cudaEventRecord(W->ev[2], st));
     CLV_CHECK(fetch_scalars(W, B, st));
 
@@ -280,6 +313,15 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     double ms_reliable = 0;
     // one BiCGStab iteration: [p update] Mhat p, alpha, s, Mhat s, omega, x/r update, rho/beta/flags, flag read-back
     auto iteration = [&](bool with_p, cudaEvent_t *kev) -> int {
+        if (merged) {  // Mhat p (+ s), Mhat s (+ omega, rho', beta), x/r/p update (+ <q0,p>, ||r||^2), alpha/flags, flag read-back
+            CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_S, r, nullptr, &grid, st, kev, nullptr, s, nullptr, W->sc_dev));
+            CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_XW, r0, W->partial, &grid, st, kev ? kev + 3 : nullptr, nullptr, nullptr, W->partial2));
+            CLV_CHECK(blas_scalar_step(bc, SC_OMEGA2, grid, tol2, delta2));
+            CLV_CHECK(blas_xrp_update<R>(bc, x, r, p, s, t, q0, &nb));
+            CLV_CHECK(blas_scalar_step(bc, SC_RHO2, nb, tol2, delta2));
+            CLV_CHECK(publish_scalars(W, B, st));
+            return 0;
+        }
         if (with_p) CLV_CHECK(blas_p_update<R>(bc, p, r, v));
         CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_W, r0, W->partial, &grid, st, kev));
         CLV_CHECK(blas_scalar_step(bc, SC_ALPHA, grid, tol2, delta2));
@@ -291,7 +333,8 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         CLV_CHECK(publish_scalars(W, B, st));
         return 0;
     };
-    if (use_graph && (!W->iter_graph || W->graph_B != B || W->graph_prec != (int)sizeof(R) || W->graph_tol2 != tol2 || W->graph_delta2 != delta2)) {
+    if (use_graph && (!W->iter_graph || W->graph_B != B || W->graph_prec != (int)sizeof(R) || W->graph_tol2 != tol2 || W->graph_delta2 != delta2 ||
+                      W->graph_merged != (int)merged)) {
         if (W->iter_graph) { cudaGraphExecDestroy(W->iter_graph); W->iter_graph = nullptr; }
         const long long nl0 = nl;
         cudaGraph_t graph = nullptr;
@@ -305,9 +348,9 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         const cudaError_t ie = cudaGraphInstantiate(&W->iter_graph, graph, 0);
         cudaGraphDestroy(graph);
         CLV_CUDA(ie);
-        W->graph_B = B; W->graph_prec = (int)sizeof(R); W->graph_tol2 = tol2; W->graph_delta2 = delta2;
+        W->graph_B = B; W->graph_prec = (int)sizeof(R); W->graph_tol2 = tol2; W->graph_delta2 = delta2; W->graph_merged = (int)merged;
     }
-    bool need_p = false;  // p = r before the first iteration
+    bool need_p = merged;  // textbook ordering: p = r before the first iteration (no p update); merged: every iteration is alike
     while (!all_done() && iters < max_iter) {
         if (use_graph && need_p) {
             CLV_CUDA(cudaGraphLaunch(W->iter_graph, st));
@@ -319,10 +362,11 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             if (!use_graph) {
                 for (int h = 0; h < 2; h++) {
                     CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h], W->kev[3 * h + 1])); ctx->stats.ms_ainv_hop += ms;
-                    CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h + 1], W->kev[3 * h + 2])); ctx->stats.ms_a_minus_hop += ms;
+                    CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[3 * h + 1], W->kev[3 * h + 2]));
+                    if (merged && h == 0) { ctx->stats.ms_a_minus_hop_s += ms; ctx->stats.n_a_minus_hop_s++; }
+                    else { ctx->stats.ms_a_minus_hop += ms; ctx->stats.n_a_minus_hop++; }
                 }
                 ctx->stats.n_ainv_hop += 2;
-                ctx->stats.n_a_minus_hop += 2;
             }
         }
         iters++;
@@ -344,10 +388,13 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         }
         {   // breakdown recovery (R11): r0 := r, rho := ||r||^2 for the rhs that asked for it; beta is already 0 so p := r next
             bool any_restart = false;
-            for (int i = 0; i < B; i++) any_restart |= !W->sc_host[i].done && W->sc_host[i].restart;
+            for (int i = 0; i < B; i++) any_restart |= !W->sc_host[i].done && W->sc_host[i].restart == 1;
             if (any_restart) {
-                CLV_CHECK(blas_restart<R>(bc, r, r0));
-                CLV_CHECK(blas_scalar_step(bc, SC_RESTART, 0, tol2, delta2));
+                if (merged) CLV_CHECK(restart_merged());
+                else {
+                    CLV_CHECK(blas_restart<R>(bc, r, r0));
+                    CLV_CHECK(blas_scalar_step(bc, SC_RESTART, 0, tol2, delta2));
+                }
             }
         }
     }

@@ -218,3 +218,26 @@ def test_solve_is_deterministic_and_reports_max_iter(B):
         res = np.linalg.norm(e[r] - oracle.apply_D(S.U, S.A, S.bc, S.kappa, p3[r])) / np.linalg.norm(e[r])
         assert 1e-10 < res < 1e-1 and abs(infos3[r]["true_resid"] - res) <= 1e-6 * res
     S.ctx.close()
+
+
+@pytest.mark.parametrize("mixed", [True, False])
+def test_merged_and_textbook_iteration_agree(B, mixed, monkeypatch):
+    """The merged ordering of the BiCGStab iteration (alpha from <Mhat^+ r0, p> before Mhat p, s written by the Dslash epilogue,
+    rho' = <r0,s> - omega <r0,t>, one x/r/p sweep; the default) and the textbook ordering (CLOVER_MERGED=0) solve the same systems:
+    both meet the oracle's residual, and their solutions agree far inside the 1e-8 parity bar."""
+    c = wl.CONFIGS[1]
+    S = Setup(B, c["dims"], c["eps"], c["kappa"], c["csw"], c["gauge_seed"])
+    eta = B.noise_fill(c["dims"], c["noise_seed"], 6, scale=wl.INV_SQRT2)   # batches 4 + 2
+    out = {}
+    for m in ("1", "0"):
+        monkeypatch.setenv("CLOVER_MERGED", m)
+        psi, infos, bad = S.ctx.solve(eta, tol=wl.TOL, batch=4, mixed=mixed)
+        assert bad == 0, infos
+        out[m] = (psi.cpu().numpy(), infos)
+    e = eta.cpu().numpy()
+    for m in ("1", "0"):
+        _check_solutions(S, e, out[m][0], out[m][1], which=[5] if m == "1" else [])
+    for r in range(6):
+        assert np.linalg.norm(out["1"][0][r] - out["0"][0][r]) / np.linalg.norm(out["0"][0][r]) < 2e-9
+        assert abs(out["1"][1][r]["iters"] - out["0"][1][r]["iters"]) <= 4
+    S.ctx.close()
