@@ -264,7 +264,7 @@ __device__ __forceinline__ bool finite_z(zs z) { return isfinite(z.re) && isfini
 // one block per rhs: sum partial[(b*B + rhs)*4 + c] over b < nblocks in a fixed order, then thread 0 updates the scalars.
 constexpr int SC_SLICES = 32;
 __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblocks, const double *__restrict__ partial, const double *__restrict__ partial2,
-                                                     RhsScalars *sc, double tol2, double delta2, double *stage, unsigned *ticket)
+                                                     RhsScalars *sc, double tol2, double delta2, double *stage, unsigned *ticket, RhsScalars *publish)
 {
     __shared__ double sm[256][7];
     __shared__ bool last;
@@ -303,21 +303,25 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         last = (atomicAdd(ticket + rhs, 1u) == SC_SLICES - 1);
     }
     __syncthreads();
-    if (!last || threadIdx.x != 0) return;
-    // stage 2 (last block of this rhs to arrive): sum the slices in order, then the scalar recurrences
+    if (!last || threadIdx.x >= 32) return;
+    // stage 2 (last block of this rhs to arrive): lane k fetches slice k (one L2 round trip for all 32 slices instead of 32
+    // dependent ones), a butterfly sums them in a fixed order, then lane 0 runs the scalar recurrences
     __threadfence();
-    ticket[rhs] = 0;
-    double d0 = 0, d1 = 0, d2 = 0, e0 = 0, e1 = 0, e2 = 0, e3 = 0;
-    for (int k = 0; k < SC_SLICES; k++) {
-        const volatile double *o = stage + ((size_t)rhs * SC_SLICES + k) * 8;
-        d0 += o[0];
-        d1 += o[1];
-        d2 += o[2];
-        e0 += o[3];
-        e1 += o[4];
-        e2 += o[5];
-        e3 += o[6];
+    static_assert(SC_SLICES == 32, "one slice per lane");
+    double e[7];
+    {
+        const volatile double *o = stage + ((size_t)rhs * SC_SLICES + threadIdx.x) * 8;
+#pragma unroll
+        for (int c = 0; c < 7; c++) e[c] = o[c];
     }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+#pragma unroll
+        for (int c = 0; c < 7; c++) e[c] += __shfl_xor_sync(0xffffffffu, e[c], off);
+    }
+    if (threadIdx.x != 0) return;
+    ticket[rhs] = 0;
+    const double d0 = e[0], d1 = e[1], d2 = e[2], e0 = e[3], e1 = e[4], e2 = e[5], e3 = e[6];
     RhsScalars &q = sc[rhs];
     const zs zero{0., 0.};
     switch (step) {
@@ -469,6 +473,13 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         q.r2 = d0 + d1;
         break;
     }
+    if (publish) {  // flag read-back without another launch: this rhs' scalars go straight into mapped pinned host memory
+        static_assert(sizeof(RhsScalars) % 8 == 0, "RhsScalars is copied in 8-byte words");
+        const unsigned long long *src = reinterpret_cast<const unsigned long long *>(&q);
+        volatile unsigned long long *dst = reinterpret_cast<volatile unsigned long long *>(publish + rhs);
+        for (int w = 0; w < (int)(sizeof(RhsScalars) / 8); w++) dst[w] = src[w];
+        __threadfence_system();
+    }
 }
 
 // ---- host wrappers ---------------------------------------------------------------------------------------
@@ -568,10 +579,10 @@ int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, cons
     CLV_CUDA(cudaGetLastError());
     return 0;
 }
-int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2)
+int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2, RhsScalars *publish)
 {
     scalar_kernel<<<dim3(c.B, SC_SLICES), 256, 0, c.st>>>(step, c.B, nblocks, c.partial, step == SC_OMEGA2 ? c.partial2 : nullptr, c.sc, tol2, delta2, c.stage,
-                                                          c.ticket);
+                                                          c.ticket, publish);
     BLAS_LAUNCHED(c);
     CLV_CUDA(cudaGetLastError());
     return 0;

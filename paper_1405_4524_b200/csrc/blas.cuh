@@ -48,6 +48,7 @@ int blas_xrp_update(const BlasCtx &c, typename Vec<R>::T *x, typename Vec<R>::T 
 template <typename R> int blas_gamma5(const BlasCtx &c, const typename Vec<R>::T *in, typename Vec<R>::T *out, int masked);
 // partial <a, b>
 template <typename R> int blas_cdot(const BlasCtx &c, const typename Vec<R>::T *a, const typename Vec<R>::T *b, int *nblocks);
-int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2);
+// `publish` (device address of mapped pinned host memory, B entries) != nullptr: each rhs' scalars are also stored there
+int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2, RhsScalars *publish = nullptr);
 
 }  // namespace clv

@@ -313,13 +313,12 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     double ms_reliable = 0;
     // one BiCGStab iteration: [p update] Mhat p, alpha, s, Mhat s, omega, x/r update, rho/beta/flags, flag read-back
     auto iteration = [&](bool with_p, cudaEvent_t *kev) -> int {
-        if (merged) {  // Mhat p (+ s), Mhat s (+ omega, rho', beta), x/r/p update (+ <q0,p>, ||r||^2), alpha/flags, flag read-back
+        if (merged) {  // Mhat p (+ s), Mhat s (+ omega, rho', beta), x/r/p update (+ <q0,p>, ||r||^2), alpha/flags + their read-back
             CLV_CHECK(mhat<R>(ctx, B, p, tmp, v, DOT_S, r, nullptr, &grid, st, kev, nullptr, s, nullptr, W->sc_dev));
             CLV_CHECK(mhat<R>(ctx, B, s, tmp, t, DOT_XW, r0, W->partial, &grid, st, kev ? kev + 3 : nullptr, nullptr, nullptr, W->partial2));
             CLV_CHECK(blas_scalar_step(bc, SC_OMEGA2, grid, tol2, delta2));
             CLV_CHECK(blas_xrp_update<R>(bc, x, r, p, s, t, q0, &nb));
-            CLV_CHECK(blas_scalar_step(bc, SC_RHO2, nb, tol2, delta2));
-            CLV_CHECK(publish_scalars(W, B, st));
+            CLV_CHECK(blas_scalar_step(bc, SC_RHO2, nb, tol2, delta2, W->sc_host_dev));   // + flag read-back (no publish launch)
             return 0;
         }
         if (with_p) CLV_CHECK(blas_p_update<R>(bc, p, r, v));
