@@ -169,11 +169,12 @@ def main():
         for prec, b in ((32, 4), (64, 8)):
             g = cfg["recon"] if prec == 32 else 18
             for nr in sorted({1, batch}):
-                for k, name, fl in ((B.KERNEL_HOP, "hop", 1320), (B.KERNEL_AINV_HOP, "ainv_hop", 1824), (B.KERNEL_A_MINUS_HOP, "a_minus_hop", 1872)):
+                for k, name, fl in ((B.KERNEL_HOP, "hop", 1320), (B.KERNEL_AINV_HOP, "ainv_hop", 1824), (B.KERNEL_A_MINUS_HOP, "a_minus_hop", 1872),
+                                    (B.KERNEL_A_MINUS_HOP_S, "a_minus_hop_s", 1872), (B.KERNEL_A_MINUS_HOP_XW, "a_minus_hop_xw", 1872)):
                     if args.kb_filter and not any(f in f"fp{prec}_{name}_b{nr}" for f in args.kb_filter.split(",")):
                         continue
                     t = ctx.bench_kernel(k, prec, nr, reps=args.reps, flush_l2=True) * 1e-3
-                    bm = (8 * g * b + (72 * b if k else 0)) / nr + 24 * b * (3 if k == B.KERNEL_A_MINUS_HOP else 2)
+                    bm = (8 * g * b + (72 * b if k else 0)) / nr + 24 * b * {B.KERNEL_A_MINUS_HOP: 3, B.KERNEL_A_MINUS_HOP_S: 4, B.KERNEL_A_MINUS_HOP_XW: 4}.get(k, 2)
                     res[f"fp{prec}_{name}_b{nr}"] = {"us": round(t * 1e6, 2), "bytes_per_site_rhs": bm, "gbs": round(bm * Vh * nr / t / 1e9, 1),
                                                      "frac_hbm": round(bm * Vh * nr / t / 1e9 / peaks["hbm_gbs"], 4), "gflops": round(fl * Vh * nr / t / 1e9, 1)}
         print(json.dumps({"kernel_bench": cfg["name"], "peak_gbs": peaks["hbm_gbs"], "kernels": res}))
@@ -238,7 +239,7 @@ def main():
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"a_minus_hop_{cfg['name']}_b{batch}")
+        traffic = json.load(open(tp)).get(f"a_minus_hop{'_xw' if merged else ''}_{cfg['name']}_b{batch}")
     epi = "t = A s - k^2 H tmp, +<t,s>,<t,t>,<r0,t>,<r0,s>" if merged else "A x - k^2 H t,+dots"
     roofline = {"bound": "hbm", "kernel": (f"dslash2_kernel<B={batch},recon={g},{epi}> (fp32, one thread per site and rhs pair)" if cfg["mixed"] and batch >= 2
                            else f"dslash_kernel<{'float' if cfg['mixed'] else 'double'},B={batch},recon={g},{epi}>"),

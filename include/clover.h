@@ -139,7 +139,10 @@ int timeslice_inner(const double *a_dev, const double *b_dev, long long n_outer,
 enum {
     CLOVER_KERNEL_HOP = 0,        /* out_e = H_eo in_o                          (1320 flop/site)  */
     CLOVER_KERNEL_AINV_HOP = 1,   /* t_o = A_oo^-1 H_oe x_e                      (1824 flop/site) */
-    CLOVER_KERNEL_A_MINUS_HOP = 2 /* y_e = A_ee x_e - kappa^2 H_eo t_o + dots    (1872 flop/site) */
+    CLOVER_KERNEL_A_MINUS_HOP = 2, /* y_e = A_ee x_e - kappa^2 H_eo t_o + <y,x>, <y,y>   (1872 flop/site) */
+    /* the two variants the merged BiCGStab iteration launches (both also read a third field w at the own site): */
+    CLOVER_KERNEL_A_MINUS_HOP_S = 3,  /* s_e = w_e - alpha (A_ee x_e - kappa^2 H_eo t_o), no reduction            */
+    CLOVER_KERNEL_A_MINUS_HOP_XW = 4  /* y_e as in 2, + <w,y>, <w,x>                                                */
 };
 /* Launch one Dslash-type kernel `reps` times back to back on internal-layout scratch fields filled with
  * pseudo-random data and return the mean device time per launch in milliseconds (CUDA events on

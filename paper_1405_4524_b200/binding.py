@@ -16,7 +16,7 @@ if not os.path.exists(LIB_PATH):
 _lib = ctypes.CDLL(LIB_PATH)
 
 OP_HOP_EO, OP_HOP_OE, OP_HOP_FULL, OP_CLOVER, OP_CLOVER_INV, OP_D_FULL, OP_MHAT = range(7)
-KERNEL_HOP, KERNEL_AINV_HOP, KERNEL_A_MINUS_HOP = range(3)
+KERNEL_HOP, KERNEL_AINV_HOP, KERNEL_A_MINUS_HOP, KERNEL_A_MINUS_HOP_S, KERNEL_A_MINUS_HOP_XW = range(5)
 EXPORTS = ["clover_create", "clover_destroy", "dslash_apply", "clover_solve", "clover_solve_host", "noise_fill",
            "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill", "timeslice_norm2", "timeslice_inner"]
 

@@ -32,6 +32,8 @@ struct SolveWork {
     void *flush = nullptr;
     cudaEvent_t ev[6] = {};
     cudaEvent_t kev[6] = {};   // per-launch timing of the two sloppy Mhat calls of an iteration: 2 x (start, mid, end)
+    cudaEvent_t kev1[2][2] = {};   // merged iteration: start / end of its first Dslash, which is queued one iteration ahead (ping-pong)
+    cudaEvent_t ev_flags = nullptr;   // merged iteration: the flags of the iteration are in host memory
     bool have_ev = false;
     // launch-bound lattices: one iteration (10 kernels + the flag read-back) replayed as a CUDA graph on an internal stream
     cudaStream_t s_work = nullptr;
@@ -60,7 +62,11 @@ void free_work(clover_ctx *ctx)
     if (W->s_in) cudaStreamDestroy(W->s_in);
     if (W->s_out) cudaStreamDestroy(W->s_out);
     cudaFree(W->flush);
-    if (W->have_ev) for (int i = 0; i < 6; i++) { cudaEventDestroy(W->ev[i]); cudaEventDestroy(W->kev[i]); }
+    if (W->have_ev) {
+        for (int i = 0; i < 6; i++) { cudaEventDestroy(W->ev[i]); cudaEventDestroy(W->kev[i]); }
+        for (int i = 0; i < 4; i++) cudaEventDestroy(W->kev1[i / 2][i % 2]);
+        cudaEventDestroy(W->ev_flags);
+    }
     if (W->iter_graph) cudaGraphExecDestroy(W->iter_graph);
     if (W->s_work) cudaStreamDestroy(W->s_work);
     if (W->ev_dep) cudaEventDestroy(W->ev_dep);
@@ -136,6 +142,8 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
     }
     if (!W->have_ev) {
         for (int i = 0; i < 6; i++) { CLV_CUDA(cudaEventCreate(&W->ev[i])); CLV_CUDA(cudaEventCreate(&W->kev[i])); }
+        for (int i = 0; i < 4; i++) CLV_CUDA(cudaEventCreate(&W->kev1[i / 2][i % 2]));
+        CLV_CUDA(cudaEventCreateWithFlags(&W->ev_flags, cudaEventDisableTiming));
         CLV_CUDA(cudaStreamCreateWithFlags(&W->s_work, cudaStreamNonBlocking));
         CLV_CUDA(cudaEventCreateWithFlags(&W->ev_dep, cudaEventDisableTiming));
         W->have_ev = true;
@@ -298,6 +306,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     // reliable update when any active rhs asks for one (delta rule), or when every active rhs claims convergence; a claim
     // that has waited 3 iterations for the others is confirmed anyway
     int claim_age = 0;
+    bool last_any_claim = false;
     auto any_update = [&]() {
         bool any_want = false, any_claim = false, all_claim = true;
         for (int i = 0; i < B; i++) {
@@ -308,6 +317,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             all_claim &= q.claim != 0;
         }
         claim_age = any_claim ? claim_age + 1 : 0;
+        last_any_claim = any_claim;
         return any_want || all_claim || claim_age >= 3;
     };
     double ms_reliable = 0;
@@ -350,8 +360,54 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         W->graph_B = B; W->graph_prec = (int)sizeof(R); W->graph_tol2 = tol2; W->graph_delta2 = delta2; W->graph_merged = (int)merged;
     }
     bool need_p = merged;  // textbook ordering: p = r before the first iteration (no p update); merged: every iteration is alike
+    // Merged iteration on lattices that are not launch-bound: its first Dslash (tmp = A^-1 H p) depends on nothing the host decides
+    // after an iteration except a restart (a reliable update changes x, y and r, never p or tmp), so the one of iteration i+1 is
+    // queued BEFORE the host waits for the flags of iteration i and the device does not idle during the round trip.  Not done while
+    // a rhs claims convergence (the batch is about to end; a speculative launch after the last iteration is merely wasted).
+    bool k1_queued = false;
+    auto dslash_k1 = [&](int e) -> int {
+        CLV_CUDA(cudaEventRecord(W->kev1[e][0], st));
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(p, nullptr, tmp, (R)1, 1, XM_NONE, 1), B, st, nullptr));
+        CLV_CUDA(cudaEventRecord(W->kev1[e][1], st));
+        nl++;
+        return 0;
+    };
+    auto iteration_after_k1 = [&]() -> int {
+        const R k2 = (R)(-ctx->kappa * ctx->kappa);
+        DslashArgs<R> a2 = dargs<R>(tmp, p, v, k2, 0, XM_CLOVER, 0, DOT_S, r, nullptr);
+        a2.out2 = s;
+        a2.sc = W->sc_dev;
+        CLV_CUDA(cudaEventRecord(W->kev[1], st));
+        CLV_CHECK(launch_dslash<R>(ctx, a2, B, st, nullptr));
+        CLV_CUDA(cudaEventRecord(W->kev[2], st));
+        CLV_CHECK(launch_dslash<R>(ctx, dargs<R>(s, nullptr, tmp, (R)1, 1, XM_NONE, 1), B, st, nullptr));
+        CLV_CUDA(cudaEventRecord(W->kev[4], st));
+        DslashArgs<R> a4 = dargs<R>(tmp, s, t, k2, 0, XM_CLOVER, 0, DOT_XW, r0, W->partial);
+        a4.partial2 = W->partial2;
+        CLV_CHECK(launch_dslash<R>(ctx, a4, B, st, &grid));
+        CLV_CUDA(cudaEventRecord(W->kev[5], st));
+        nl += 3;
+        CLV_CHECK(blas_scalar_step(bc, SC_OMEGA2, grid, tol2, delta2));
+        CLV_CHECK(blas_xrp_update<R>(bc, x, r, p, s, t, q0, &nb));
+        CLV_CHECK(blas_scalar_step(bc, SC_RHO2, nb, tol2, delta2, W->sc_host_dev));
+        CLV_CUDA(cudaEventRecord(W->ev_flags, st));
+        return 0;
+    };
     while (!all_done() && iters < max_iter) {
-        if (use_graph && need_p) {
+        if (merged && !use_graph) {
+            const int e = iters & 1;
+            if (!k1_queued) CLV_CHECK(dslash_k1(e));
+            CLV_CHECK(iteration_after_k1());
+            k1_queued = !last_any_claim && iters + 1 < max_iter;
+            if (k1_queued) CLV_CHECK(dslash_k1(e ^ 1));
+            CLV_CUDA(cudaEventSynchronize(W->ev_flags));
+            clover_solve_stats &S = ctx->stats;
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev1[e][0], W->kev1[e][1])); S.ms_ainv_hop += ms;
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[2], W->kev[4])); S.ms_ainv_hop += ms;
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[1], W->kev[2])); S.ms_a_minus_hop_s += ms;
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[4], W->kev[5])); S.ms_a_minus_hop += ms;
+            S.n_ainv_hop += 2; S.n_a_minus_hop_s++; S.n_a_minus_hop++;
+        } else if (use_graph && need_p) {
             CLV_CUDA(cudaGraphLaunch(W->iter_graph, st));
             nl += W->graph_kernels;
             CLV_CUDA(cudaStreamSynchronize(st));
@@ -389,7 +445,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             bool any_restart = false;
             for (int i = 0; i < B; i++) any_restart |= !W->sc_host[i].done && W->sc_host[i].restart == 1;
             if (any_restart) {
-                if (merged) CLV_CHECK(restart_merged());
+                if (merged) { CLV_CHECK(restart_merged()); k1_queued = false; }   // p changed, tmp was scratch
                 else {
                     CLV_CHECK(blas_restart<R>(bc, r, r0));
                     CLV_CHECK(blas_scalar_step(bc, SC_RESTART, 0, tol2, delta2));
@@ -600,6 +656,15 @@ template <typename R> static int bench_impl(clover_ctx *ctx, int kernel, int B, 
     case CLOVER_KERNEL_HOP: a = dargs<R>(f[0], nullptr, f[3], (R)1, 0, XM_NONE, 0); break;
     case CLOVER_KERNEL_AINV_HOP: a = dargs<R>(f[0], nullptr, f[3], (R)1, 1, XM_NONE, 1); break;
     case CLOVER_KERNEL_A_MINUS_HOP: a = dargs<R>(f[0], f[1], f[3], k2, 0, XM_CLOVER, 0, DOT_X, nullptr, W->partial); break;
+    case CLOVER_KERNEL_A_MINUS_HOP_S:
+        a = dargs<R>(f[0], f[1], f[3], k2, 0, XM_CLOVER, 0, DOT_S, f[2]);
+        a.out2 = f[3];
+        a.sc = W->sc_dev;
+        break;
+    case CLOVER_KERNEL_A_MINUS_HOP_XW:
+        a = dargs<R>(f[0], f[1], f[3], k2, 0, XM_CLOVER, 0, DOT_XW, f[2], W->partial);
+        a.partial2 = W->partial2;
+        break;
     default: set_error("clover_bench_kernel: unknown kernel %d", kernel); return CLOVER_EINVAL;
     }
     double total = 0;

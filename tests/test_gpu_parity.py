@@ -164,7 +164,7 @@ def test_solve_ragged_batches_and_dilution_recon12(B):
     S.ctx.close()
 
 
-def test_solve_point_source_free_field(B):
+def test_solve_point_source_free_field(B, monkeypatch):
     """Unit links, delta sources: <r0, v> vanishes exactly in the second iteration; the solver restarts with r0 := r (R11),
     as the oracle does, and still reaches the tolerance.  Checked against the oracle's solve and its D."""
     dims = (4, 4, 4, 8)
@@ -174,7 +174,9 @@ def test_solve_point_source_free_field(B):
     eta[0, 0, 0, 0, 0, 2, 1] = 1
     eta[1, 3, 1, 2, 3, 0, 0] = 1
     A = oracle.clover_matrix(U, 0.12, 1.0)
-    for mixed in (True, False):
+    for mixed, graph in ((True, None), (False, None), (True, "0")):   # "0": launch-by-launch path (restart with a Dslash queued ahead)
+        if graph is not None:
+            monkeypatch.setenv("CLOVER_GRAPH", graph)
         psi, infos, bad = ctx.solve(dev(eta), tol=1e-10, batch=2, mixed=mixed)
         assert bad == 0, infos
         for r in range(2):
@@ -234,6 +236,13 @@ def test_merged_and_textbook_iteration_agree(B, mixed, monkeypatch):
         psi, infos, bad = S.ctx.solve(eta, tol=wl.TOL, batch=4, mixed=mixed)
         assert bad == 0, infos
         out[m] = (psi.cpu().numpy(), infos)
+    # the launch-by-launch path of large lattices (no CUDA graph; the next iteration's first Dslash queued ahead of the flag
+    # read-back) runs the same arithmetic in the same order as the graph replay: bit-identical solutions
+    monkeypatch.setenv("CLOVER_MERGED", "1")
+    monkeypatch.setenv("CLOVER_GRAPH", "0")
+    psi, infos, bad = S.ctx.solve(eta, tol=wl.TOL, batch=4, mixed=mixed)
+    assert bad == 0 and np.array_equal(psi.cpu().numpy(), out["1"][0]) and infos == out["1"][1]
+    monkeypatch.delenv("CLOVER_GRAPH")
     e = eta.cpu().numpy()
     for m in ("1", "0"):
         _check_solutions(S, e, out[m][0], out[m][1], which=[5] if m == "1" else [])
