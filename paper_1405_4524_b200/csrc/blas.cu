@@ -469,6 +469,15 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             q.alpha = st_z(al);
         }
         break;
+    case SC_CONFIRM:  // d0 + d1 = ||eta - D psi||^2 on the full lattice, computed because every active rhs claimed convergence
+        q.claim = 0;
+        if (!q.done) {
+            const double f = d0 + d1;
+            if (!isfinite(f)) { q.done = 1; q.status = 3; }
+            else if (f <= tol2 * q.eta2) { q.done = 1; q.true_r2 = f; q.alpha = q.beta = q.gam = st_z(zero); }
+        }
+        if (q.done) q.r2 = d0 + d1;  // (a rhs that failed keeps its iterated ||r||^2; the reliable update that follows replaces it)
+        break;
     case SC_FINAL:  // d0 + d1 = ||eta - D psi||^2 on the full lattice; stored in r2 (true_r2 keeps the even-odd value)
         q.r2 = d0 + d1;
         break;

@@ -37,7 +37,8 @@ int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, cons
 
 // scalar steps (one block per rhs): reduce the partials of `nblocks` blocks and update RhsScalars
 enum { SC_ETA2 = 0, SC_INIT = 1, SC_ALPHA = 2, SC_OMEGA = 3, SC_RHO = 4, SC_TRUE = 5, SC_FINAL = 6, SC_RESTART = 7,
-       SC_INIT_MERGED = 8, SC_OMEGA2 = 9, SC_RHO2 = 10, SC_RESTART2 = 11 };  // merged iteration (solver.cu)
+       SC_INIT_MERGED = 8, SC_OMEGA2 = 9, SC_RHO2 = 10, SC_RESTART2 = 11,  // merged iteration (solver.cu)
+       SC_CONFIRM = 12 };  // full-lattice verification that also decides convergence
 // r0 = r for the rhs whose `restart` flag is set (breakdown recovery)
 template <typename R> int blas_restart(const BlasCtx &c, const typename Vec<R>::T *r, typename Vec<R>::T *r0, typename Vec<R>::T *p = nullptr);
 // merged iteration: x += alpha p + omega s ; r' = s - omega t ; p = r' + beta p - gam (r - s) ; partial <q0,p>, ||r'||^2

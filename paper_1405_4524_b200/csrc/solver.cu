@@ -306,7 +306,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     // reliable update when any active rhs asks for one (delta rule), or when every active rhs claims convergence; a claim
     // that has waited 3 iterations for the others is confirmed anyway
     int claim_age = 0;
-    bool last_any_claim = false;
+    bool last_any_claim = false, last_all_claim = false;
     auto any_update = [&]() {
         bool any_want = false, any_claim = false, all_claim = true;
         for (int i = 0; i < B; i++) {
@@ -318,9 +318,27 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         }
         claim_age = any_claim ? claim_age + 1 : 0;
         last_any_claim = any_claim;
+        last_all_claim = all_claim;
         return any_want || all_claim || claim_age >= 3;
     };
-    double ms_reliable = 0;
+    double ms_reliable = 0, ms_confirm = 0;
+    bool verified = false;
+    // odd sites and verification on the full lattice, all fp64: psi_o = A_oo^-1 (eta_o + kappa H_oe y), then ||eta - D psi||^2 out of
+    // the epilogues of the two Dslash launches that apply D (residual variant without a store), their per-block partials reduced
+    // together by the scalar step (SC_FINAL: report; SC_CONFIRM: also decide convergence)
+    auto verify = [&](int step) -> int {
+        CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, eta_o, psi_o, ctx->kappa, 1, XM_PLAIN, 1), B, st, nullptr));
+        CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(psi_o, y, nullptr, -ctx->kappa, 0, XM_CLOVER, 0, DOT_RES, eta_e, W->partial), B, st, &grid));
+        if (2 * grid > W->partial_blocks) {
+            set_error("solve: partial buffer too small for the verification (%d blocks)", grid);
+            return CLOVER_EINVAL;
+        }
+        CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, psi_o, nullptr, -ctx->kappa, 1, XM_CLOVER, 0, DOT_RES, eta_o, W->partial + (size_t)grid * B * 4), B,
+                                        st, nullptr));
+        nl += 3;
+        CLV_CHECK(blas_scalar_step(bc, step, 2 * grid, tol2, delta2));
+        return 0;
+    };
     // one BiCGStab iteration: [p update] Mhat p, alpha, s, Mhat s, omega, x/r update, rho/beta/flags, flag read-back
     auto iteration = [&](bool with_p, cudaEvent_t *kev) -> int {
         if (merged) {  // Mhat p (+ s), Mhat s (+ omega, rho', beta), x/r/p update (+ <q0,p>, ||r||^2), alpha/flags + their read-back
@@ -430,6 +448,18 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             // reliable update: y += x, x = 0, r = b - Mhat y in fp64 (S 8(c) O6')
             CLV_CUDA(cudaEventRecord(W->ev[4], st));
             CLV_CHECK(blas_accumulate_y<R>(bc, y, x));
+            if (last_all_claim && iters < max_iter) {
+                // every active rhs claims convergence: confirm it with what the solve ends with anyway -- the odd sites and the fp64
+                // residual on the full lattice (with exact odd sites it IS the even-odd residual (b - Mhat y, 0), R10) -- instead of
+                // an even-odd recomputation followed by the same verification.  A rhs that fails goes on with a reliable update.
+                CLV_CHECK(verify(SC_CONFIRM));
+                CLV_CUDA(cudaEventRecord(W->ev[5], st));
+                CLV_CHECK(fetch_scalars(W, B, st));
+                CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[4], W->ev[5]));
+                ms_confirm += ms;
+                if (all_done()) { verified = true; updates++; break; }
+                CLV_CUDA(cudaEventRecord(W->ev[4], st));
+            }
             // r = b - Mhat y with ||r||^2, fused into the epilogue of the second fp64 Dslash and stored in the iteration precision
             CLV_CHECK(mhat<double>(ctx, B, y, tmp64, sizeof(R) == 8 ? (double2 *)r : nullptr, DOT_RES, b, W->partial, &grid, st, nullptr,
                                    sizeof(R) == 4 ? (float4 *)r : nullptr));
@@ -454,18 +484,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         }
     }
     CLV_CUDA(cudaEventRecord(W->ev[3], st));
-    // odd sites and verification on the full lattice, all fp64: ||eta - D psi||^2 comes out of the epilogues of the two Dslash
-    // launches that apply D (residual variant without a store), their per-block partials reduced together
-    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, eta_o, psi_o, ctx->kappa, 1, XM_PLAIN, 1), B, st, nullptr));
-    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(psi_o, y, nullptr, -ctx->kappa, 0, XM_CLOVER, 0, DOT_RES, eta_e, W->partial), B, st, &grid));
-    if (2 * grid > W->partial_blocks) {
-        set_error("solve: partial buffer too small for the verification (%d blocks)", grid);
-        return CLOVER_EINVAL;
-    }
-    CLV_CHECK(launch_dslash<double>(ctx, dargs<double>(y, psi_o, nullptr, -ctx->kappa, 1, XM_CLOVER, 0, DOT_RES, eta_o, W->partial + (size_t)grid * B * 4), B, st,
-                                    nullptr));
-    nl += 3;
-    CLV_CHECK(blas_scalar_step(bc, SC_FINAL, 2 * grid, tol2, delta2));
+    if (!verified) CLV_CHECK(verify(SC_FINAL));
     CLV_CUDA(cudaEventRecord(W->ev[4], st));
     CLV_CHECK((reorder_out<double, double>(g, dst, y, psi_o, B, st)));
     nl++;
@@ -476,9 +495,9 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[0], W->ev[1])); S.ms_reorder += ms;
     CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[4], W->ev[5])); S.ms_reorder += ms;
     CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[1], W->ev[2])); S.ms_prep += ms;
-    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[2], W->ev[3])); S.ms_iterate += ms - ms_reliable;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[2], W->ev[3])); S.ms_iterate += ms - ms_reliable - ms_confirm;
     S.ms_reliable += ms_reliable;
-    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[3], W->ev[4])); S.ms_finish += ms;
+    CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[3], W->ev[4])); S.ms_finish += ms + ms_confirm;
     CLV_CUDA(cudaEventElapsedTime(&ms, W->ev[0], W->ev[5])); S.ms_total += ms;
 
     int bad = 0;
