@@ -222,7 +222,10 @@ static double reliable_delta()
 {
     const char *e = getenv("CLOVER_DELTA");  // tuning/debug knob only
     const double d = e ? atof(e) : 0.0;
-    return (d > 0.0 && d < 1.0) ? d : 1e-4;
+    // 3e-6: two fp32 legs (1 -> 3e-6 -> 1e-10 relative to ||eta||), each well inside what fp32 recurrences resolve (the iterated
+    // residual of a leg is good to ~1e-6 of the leg's start); measured at 24^3x48: 1e-4..1e-5 three fp64 recomputations per batch,
+    // 3e-6 two with the same iteration count, 1e-6 two with one more iteration (profiles/r1_tuning.md)
+    return (d > 0.0 && d < 1.0) ? d : 3e-6;
 }
 
 // Small lattices are launch-bound (a 16^3x32 Dslash takes ~10 us): replay the iteration as a CUDA graph there.
