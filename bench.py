@@ -380,7 +380,9 @@ def main():
            "config": {"workload": cfg["name"], "n_rhs_per_gpu": n_rhs, "batch": batch, "tol": wl.TOL, "kappa": cfg["kappa"], "c_sw": cfg["csw"],
                       "eps": cfg["eps"], "recon": cfg["recon"], "time_dilution": cfg["dilution"],
                       "solver": "even-odd BiCGStab, fp32 iteration + fp64 reliable updates" if cfg["mixed"] else "even-odd BiCGStab fp64",
-                      "l2": "fields per sweep (>= 255 MB at batch 8) exceed the 126 MB L2; the stand-alone hop timing flushes L2 between launches"},
+                      "l2": ("one fp32 field of the batch is %.0f MB; " % (Vh * batch * 96 / 1e6)) +
+                            ("fields per sweep exceed the 126 MB L2; " if Vh * batch * 96 * 3 > 126e6 else "the sweeps FIT the 126 MB L2 (parity-size lattice: HBM fractions are not meaningful here); ") +
+                            "the stand-alone hop timing flushes L2 between launches"},
            "clocks": sampler.summary(), "gpu_launches": launches, "roofline": roofline, "dslash": dslash, "e2e": e2e, "noise_fill": noise, "next_contraction": contraction, "next_fill": fill_res,
            "solve": {"iters": [i["iters"] for i in last["infos"]][::batch], "reliable_updates": [i["reliable_updates"] for i in last["infos"]][::batch],
                      "max_true_resid": max(i["true_resid"] for i in last["infos"]),
