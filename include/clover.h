@@ -55,7 +55,8 @@ typedef struct {
     int status;           /* 0 converged, 1 max_iter reached, 2 repeated breakdown (<r0,v> = 0 after 8 restarts), 3 non-finite */
     int iters;            /* BiCGStab iterations of the batch this source was in */
     int reliable_updates; /* fp64 residual recomputations of that batch */
-    double iter_resid;    /* last fp64 even-odd residual ||b_e - Mhat y|| / ||eta|| */
+    double iter_resid;    /* the fp64 residual the convergence decision was taken on: ||b_e - Mhat y|| / ||eta|| of the last reliable
+                             update, or the full-lattice residual when the final verification confirmed the claim itself */
     double true_resid;    /* full-lattice fp64 ||eta - D psi|| / ||eta||, recomputed from the returned psi */
 } clover_rhs_info;
 
@@ -85,6 +86,8 @@ int dslash_apply(clover_ctx *ctx, int op, int precision, const void *in_dev, voi
 /* Solve D psi_r = eta_r, r = 0..n_rhs-1, canonical fp64 in and out (device), by even-odd
  * preconditioned BiCGStab batched `batch` right-hand sides per Dslash launch (1, 2, 4 or 8, <= max_rhs):
  * mixed = 1: fp32 iteration with fp64 reliable updates (S 8(c) O6'); mixed = 0: everything fp64.
+ * The iteration is the textbook recurrence with its dot products re-ordered (alpha from <Mhat^+ r0, p>, rho' from <r0,s> - omega <r0,t>;
+ * DESIGN.md sec. 1) so that the BLAS-1 streams ride in the Dslash epilogues; results differ from the textbook ordering by rounding only.
  * Stops when the fp64 residual ||eta - D psi|| / ||eta|| <= tol (R10).  info_host: n_rhs entries, host.
  * Synchronises `stream`.  Returns the number of non-converged sources (0 = all good) or CLOVER_E*. */
 int clover_solve(clover_ctx *ctx, const double *sources_dev, double *propagators_dev, int n_rhs, double tol,
