@@ -221,7 +221,7 @@ __global__ void __launch_bounds__(BLAS_BLOCK) residual_kernel(size_t n64, int B,
             v.x -= ww.x;
             v.y -= ww.y;
         }
-        r64[i] = v;
+        if (r64) r64[i] = v;
         store_sloppy(rs, i, v);
         d0 += norm2(v);
     }

@@ -30,7 +30,7 @@ int blas_xr_update(const BlasCtx &c, typename Vec<R>::T *x, typename Vec<R>::T *
 template <typename R> int blas_p_update(const BlasCtx &c, typename Vec<R>::T *p, const typename Vec<R>::T *r, const typename Vec<R>::T *v);
 // y += x (fp64 accumulate), x = 0
 template <typename R> int blas_accumulate_y(const BlasCtx &c, double2 *y, typename Vec<R>::T *x);
-// r64 = b - w (w may be null: r64 = b) ; rs = (R) r64 ; partial ||r64||^2
+// r64 = b - w (w may be null: r64 = b; r64 itself may be null: not stored) ; rs = (R) r64 ; partial ||r64||^2
 template <typename R> int blas_residual(const BlasCtx &c, const double2 *b, const double2 *w, double2 *r64, typename Vec<R>::T *rs, int *nblocks);
 // partial d0 = ||a1 - b1||^2, d1 = ||a2 - b2||^2 (b1, b2 may be null)
 int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, const double2 *a2, const double2 *b2, int *nblocks);

@@ -259,7 +259,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         CLV_CUDA(cudaEventRecord(W->ev_dep, st_user));
         CLV_CUDA(cudaStreamWaitEvent(st, W->ev_dep, 0));
     }
-    double2 *eta_e = W->f64[F_ETA_E], *eta_o = W->f64[F_ETA_O], *b = W->f64[F_B], *y = W->f64[F_Y], *r64 = W->f64[F_R64],
+    double2 *eta_e = W->f64[F_ETA_E], *eta_o = W->f64[F_ETA_O], *b = W->f64[F_B], *y = W->f64[F_Y],
             *tmp64 = W->f64[F_TMP64], *psi_o = W->f64[F_PSI_O];
     V *x = (V *)W->sl[S_X], *r = (V *)W->sl[S_R], *p = (V *)W->sl[S_P], *v = (V *)W->sl[S_V], *s = (V *)W->sl[S_S], *t = (V *)W->sl[S_T],
       *r0 = (V *)W->sl[S_R0], *tmp = (V *)W->sl[S_TMP], *q0 = (V *)W->sl[S_Q0];
@@ -284,7 +284,7 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
     // y = 0, x = 0, r = b, p = r0 = r
     CLV_CUDA(cudaMemsetAsync(y, 0, nbytes64, st));
     CLV_CUDA(cudaMemsetAsync(x, 0, nbytes, st));
-    CLV_CHECK(blas_residual<R>(bc, b, nullptr, r64, r, &nb));
+    CLV_CHECK(blas_residual<R>(bc, b, nullptr, nullptr, r, &nb));   // r = (R) b, ||b||^2; no fp64 copy of r is kept
     CLV_CHECK(blas_scalar_step(bc, merged ? SC_INIT_MERGED : SC_INIT, nb, tol2, delta2));
     // merged iteration, (re)start of the rhs flagged `restart == 1`: r0 := p := r, q0 := Mhat^+ r0 = gamma5 Mhat gamma5 r0,
     // rho := ||r||^2, alpha := rho / <q0, p>.  s, t and tmp are free between iterations and serve as scratch.
