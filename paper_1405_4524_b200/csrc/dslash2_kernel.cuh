@@ -18,6 +18,9 @@ namespace clv {
 #ifndef CLV_R2_BLOCK_NODOT
 #define CLV_R2_BLOCK_NODOT 32   // threads per CTA of the pair-kernel variants without dot products
 #endif
+#ifndef CLV_R2_BLOCK_DOT
+#define CLV_R2_BLOCK_DOT 64   // threads per CTA of the pair-kernel variants that write a line of partial sums per CTA (128: +4 us per launch; 32: four times the lines for the scalar kernels, slower overall)
+#endif
 #ifndef CLV_R2_SMEM
 #define CLV_R2_SMEM 1   // stage the CTA's clover blocks in shared memory with cp.async at kernel start
 #endif

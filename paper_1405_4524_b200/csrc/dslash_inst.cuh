@@ -15,13 +15,13 @@ static int launch_dslash2_BR(const clover_ctx *ctx, const OpData<float> &op, con
 {
     const Geom &g = ctx->geom;
     const unsigned npairs = (unsigned)g.Vh * B / 2;
-    const unsigned block = CLV_HAS_RED(a.dot) ? DSLASH_BLOCK : CLV_R2_BLOCK_NODOT;
+    const unsigned block = CLV_HAS_RED(a.dot) ? CLV_R2_BLOCK_DOT : CLV_R2_BLOCK_NODOT;
     const unsigned grid = (npairs + block - 1) / block;
     if (grid_out) *grid_out = (int)grid;
     const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
 #define CLV_LAUNCH2(XM, PI, DT)                                                      \
     case (XM) * 100 + (PI) * 10 + (DT):                                              \
-        dslash2_kernel<B, RECON, XM, PI, DT, (CLV_HAS_RED(DT) ? DSLASH_BLOCK : CLV_R2_BLOCK_NODOT)><<<grid, block, 0, st>>>(g, op, a); \
+        dslash2_kernel<B, RECON, XM, PI, DT, (CLV_HAS_RED(DT) ? CLV_R2_BLOCK_DOT : CLV_R2_BLOCK_NODOT)><<<grid, block, 0, st>>>(g, op, a); \
         break;
     switch (key) {
         CLV_LAUNCH2(XM_NONE, 0, DOT_NONE)
