@@ -5,8 +5,9 @@ A step = one pass of the whole hot path over one batch of synthetic input at BAS
 (24^3x48, kappa 0.118, c_sw 1.5, links exp(i 0.4 H)): noise_fill of N_r = 32 Z4 sources, then clover_solve of all of
 them in batches of 8 (fp32 BiCGStab with fp64 reliable updates, tol 1e-10), source prep, odd-site reconstruction,
 fp64 full-lattice verification and layout reorders included.  metric = BiCGStab seconds/source; the Dslash GB/s half
-of BASELINE.json's metric is the `roofline` object (the fused fp32 Dslash kernel of the iteration, timed launch by
-launch with CUDA events inside the timed steps) plus `dslash` (the plain hop kernel timed alone).
+of BASELINE.json's metric is the `roofline` object (the kernel of the iteration with the largest summed device time, every
+launch timed with CUDA events inside the timed steps; the other kernels under `other_kernels`) plus `dslash` (the plain hop
+kernel timed alone).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config i]
 """
@@ -71,46 +72,72 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s)}
 
 
-def oracle_sample(cfg, iters_sample, U=None):
-    """Time the CPU oracle as it stands on a bounded sample: `iters_sample` BiCGStab iterations of one source on the full
-    lattice, scaled by the iteration count the same oracle needs to reach 1e-10 with the same parameters on 8^3x16
-    (iteration counts are volume independent for these uncorrelated links)."""
-    import numpy as np
+def oracle_setup(cfg, U=None):
     import oracle
     from paper_1405_4524_b200 import workloads as wl
-    small = (8, 8, 8, 16)
-    Us = wl.gauge_links(small, cfg["eps"], cfg["gauge_seed"])
-    As = oracle.clover_matrix(Us, cfg["kappa"], cfg["csw"])
-    _, info = oracle.bicgstab(Us, As, wl.BC, cfg["kappa"], oracle.noise_fill(small, cfg["noise_seed"], 1, scale=wl.INV_SQRT2)[0], tol=wl.TOL)
-    n_it = info["iters"]
     if U is None:
         U = wl.gauge_links(cfg["dims"], cfg["eps"], cfg["gauge_seed"])
     A = oracle.clover_matrix(U, cfg["kappa"], cfg["csw"])
-    eta = oracle.noise_fill(cfg["dims"], cfg["noise_seed"], 1, scale=wl.INV_SQRT2)[0]
+    eta = oracle.noise_fill(cfg["dims"], cfg["noise_seed"], 1, time_dilution=cfg["dilution"], scale=wl.INV_SQRT2)[0]
+    return oracle, wl, U, A, eta
 
-    def run():
-        t0 = time.perf_counter()
-        oracle.bicgstab(U, A, wl.BC, cfg["kappa"], eta, tol=1e-30, max_iter=iters_sample)
-        return (time.perf_counter() - t0) / iters_sample * n_it   # seconds per source
-    return run, n_it, oracle.threads()
+
+def oracle_full_solve(cfg, U=None):
+    """cpu_baseline: ONE full solve of one source of the workload by the oracle as it stands (unpreconditioned fp64 BiCGStab to
+    the workload's tolerance, all host cores), measured, plus the oracle's D-apply rate on all cores and on one thread."""
+    oracle, wl, U, A, eta = oracle_setup(cfg, U)
+    cores = oracle.threads()
+    t0 = time.perf_counter()
+    _, info = oracle.bicgstab(U, A, wl.BC, cfg["kappa"], eta, tol=wl.TOL)
+    t_solve = time.perf_counter() - t0
+    sites = eta.size // 12
+
+    def d_rate(threads, reps):
+        oracle.set_threads(threads)
+        oracle.apply_D(U, A, wl.BC, cfg["kappa"], eta)
+        t = time.perf_counter()
+        for _ in range(reps):
+            oracle.apply_D(U, A, wl.BC, cfg["kappa"], eta)
+        dt = (time.perf_counter() - t) / reps
+        oracle.set_threads(cores)
+        return {"threads": threads, "s_per_apply": dt, "sites_per_s": sites / dt, "gflops": 1872.0 * sites / dt / 1e9}
+    return {"value": t_solve, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"full solve of 1 source of {cfg['name']} to {wl.TOL:g}: {info['iters']} iterations of the oracle's unpreconditioned fp64 BiCGStab "
+                      f"(2 D applies each), true residual {info['true_resid']:.2e}, measured not projected",
+            "iters": info["iters"], "true_resid": info["true_resid"], "extrapolated": False,
+            "d_apply": {"flop_per_site": 1872, "all_cores": d_rate(cores, 3), "one_thread": d_rate(1, 1)}}
 
 
 def run_reference(args, cfg):
-    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    """--impl reference: the oracle on the host cores (rank 0 only).  One full solve first (its iteration count N and measured
+    time are reported in cpu_baseline); every timed step then measures the oracle's cost per BiCGStab iteration on the same
+    source as the difference between a 10-iteration and a 2-iteration call (so the set-up and the trailing true-residual apply
+    of a call cancel) and reports N x that: a bounded sample of the same work, kept in line with the full solve."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    iters_sample = 2
-    run, n_it, cores = oracle_sample(cfg, iters_sample)
+    base = oracle_full_solve(cfg)
+    oracle, wl, U, A, eta = oracle_setup(cfg)
+    n_it, lo, hi = base["iters"], 2, 10
+
+    def call(n):
+        t0 = time.perf_counter()
+        oracle.bicgstab(U, A, wl.BC, cfg["kappa"], eta, tol=1e-30, max_iter=n)
+        return time.perf_counter() - t0
+
+    def run():
+        return (call(hi) - call(lo)) / (hi - lo) * n_it   # seconds per source
     for _ in range(args.warmup):
         run()
     vals = [run() for _ in range(args.steps)]
     v = sum(vals) / len(vals)
-    sample = (f"{iters_sample} BiCGStab iterations (2 D applies each + true residual) of 1 source on {cfg['name']}, "
-              f"scaled to the {n_it} iterations the oracle needs for 1e-10 at these parameters on 8^3x16")
+    base["per_iteration_s_full_solve"] = base["value"] / n_it
+    base["per_iteration_s_sampled"] = v / n_it
+    base["sample"] += (f"; each timed step of this arm = ({hi}-iteration call - {lo}-iteration call) / {hi - lo} x {n_it} iterations on the same source")
+    base["value"] = v
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": v * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f64", "data": "synthetic", "config": {"workload": cfg["name"], "n_rhs": 1, "solver": "oracle BiCGStab, unpreconditioned"},
-                      "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                      "cpu_baseline": base,
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
@@ -185,7 +212,8 @@ def main():
     eta = torch.empty((n_rhs, T, Z, Y, X, 4, 3), dtype=torch.complex128, device="cuda")
     psi = torch.empty_like(eta)
     launches = 0
-    kstats = {"n_ainv_hop": 0, "n_a_minus_hop": 0, "ms_ainv_hop": 0.0, "ms_a_minus_hop": 0.0, "n_a_minus_hop_s": 0, "ms_a_minus_hop_s": 0.0}
+    kstats = {"n_ainv_hop": 0, "n_a_minus_hop": 0, "ms_ainv_hop": 0.0, "ms_a_minus_hop": 0.0, "n_a_minus_hop_s": 0, "ms_a_minus_hop_s": 0.0,
+              "n_xrp_update": 0, "ms_xrp_update": 0.0}
     phases = {k: 0.0 for k in ("ms_total", "ms_reorder", "ms_prep", "ms_iterate", "ms_reliable", "ms_finish")}
     last = {}
 
@@ -219,41 +247,56 @@ def main():
     ms = max_over_ranks(e0.elapsed_time(e1))
     value = sharding.whole_job_seconds_per_source(ms, args.steps, n_rhs, world)   # world * n_rhs sources per step
 
-    # ---- roofline of the dominant kernel: the fused fp32 Dslash y_e = A x_e - kappa^2 H_eo t_o (+dots) of the iteration ----
+    # ---- roofline of the DOMINANT kernel: the kernel of the solve with the largest summed device time inside the timed steps
+    # (clover_get_stats: CUDA events around every launch on the solve's stream); the others are listed under other_kernels ----
     peaks, peak_kind = measured_peaks()
     b = 4 if cfg["mixed"] else 8
     g = cfg["recon"] if cfg["mixed"] else 18
     merged = kstats["n_a_minus_hop_s"] > 0   # merged iteration (solver.cu): both fused Dslash variants also read w (r or r0) at the own site
     bytes_a_minus = (8 * g * b + 72 * b) / batch + 24 * b * (4 if merged else 3)   # links + clover shared by the batch; in, x, (w,) out per rhs
     bytes_ainv = (8 * g * b + 72 * b) / batch + 24 * b * 2
+    bytes_xrp = 24 * b * 9      # one sweep: reads x, p, s, t, r, q0, writes x, r, p
     prec = 32 if cfg["mixed"] else 64
+    rt, pair = ("float" if cfg["mixed"] else "double"), (cfg["mixed"] and batch >= 2)
+    kname = (lambda what: f"dslash2_kernel<B={batch},recon={g},{what}> (fp32, one thread per site and rhs pair)") if pair else \
+            (lambda what: f"dslash_kernel<{rt},B={batch},recon={g},{what}>")
     timed = "CUDA events around every launch inside the timed steps"
+    table = {}   # name -> (kernel, launches, summed ms, algorithmic bytes / site / rhs, flop / site / rhs, traffic key)
     if kstats["n_a_minus_hop"]:
-        t_a_minus = kstats["ms_a_minus_hop"] / kstats["n_a_minus_hop"] * 1e-3
-        t_ainv = kstats["ms_ainv_hop"] / kstats["n_ainv_hop"] * 1e-3
+        table["ainv_hop"] = (kname("tmp = A^-1 H x"), kstats["n_ainv_hop"], kstats["ms_ainv_hop"], bytes_ainv, 1824.0, "ainv_hop")
+        table["a_minus_hop"] = (kname("t = A s - k^2 H tmp, +<t,s>,<t,t>,<r0,t>,<r0,s>" if merged else "A x - k^2 H t,+dots"), kstats["n_a_minus_hop"],
+                                kstats["ms_a_minus_hop"], bytes_a_minus, 1872.0, "a_minus_hop_xw" if merged else "a_minus_hop")
+        if merged:
+            table["a_minus_hop_s"] = (kname("s = r - alpha (A p - k^2 H tmp)"), kstats["n_a_minus_hop_s"], kstats["ms_a_minus_hop_s"], bytes_a_minus, 1872.0,
+                                      "a_minus_hop_s")
+            if kstats["n_xrp_update"]:
+                table["xrp_update"] = (f"xrp_update_kernel<{rt}> (x, r, p updates + <q0,p>, ||r||^2: 9 vector passes)", kstats["n_xrp_update"],
+                                       kstats["ms_xrp_update"], bytes_xrp, 0.0, "xrp_update")
     else:   # launch-bound lattice: the iteration ran as a CUDA graph, without per-launch events; time the kernels alone
-        t_a_minus = ctx.bench_kernel(B.KERNEL_A_MINUS_HOP, prec, batch, reps=20) * 1e-3
-        t_ainv = ctx.bench_kernel(B.KERNEL_AINV_HOP, prec, batch, reps=20) * 1e-3
         timed = "kernel timed alone (the solve replays its iteration as a CUDA graph on this lattice; fields fit L2)"
-    ach = bytes_a_minus * Vh * batch / t_a_minus / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
+        table["ainv_hop"] = (kname("tmp = A^-1 H x"), 20, ctx.bench_kernel(B.KERNEL_AINV_HOP, prec, batch, reps=20) * 20, bytes_ainv, 1824.0, "ainv_hop")
+        table["a_minus_hop"] = (kname("A x - k^2 H t,+dots"), 20, ctx.bench_kernel(B.KERNEL_A_MINUS_HOP, prec, batch, reps=20) * 20, bytes_a_minus, 1872.0, "a_minus_hop")
+    traffic_db, tp = {}, os.path.join(ROOT, "profiles", "traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"a_minus_hop{'_xw' if merged else ''}_{cfg['name']}_b{batch}")
-    epi = "t = A s - k^2 H tmp, +<t,s>,<t,t>,<r0,t>,<r0,s>" if merged else "A x - k^2 H t,+dots"
-    roofline = {"bound": "hbm", "kernel": (f"dslash2_kernel<B={batch},recon={g},{epi}> (fp32, one thread per site and rhs pair)" if cfg["mixed"] and batch >= 2
-                           else f"dslash_kernel<{'float' if cfg['mixed'] else 'double'},B={batch},recon={g},{epi}>"),
-                "achieved": ach, "timed": timed, "peak": peaks["hbm_gbs"], "peak_kind": peak_kind, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
-                "traffic": traffic, "algorithmic_bytes_per_site_rhs": bytes_a_minus, "us_per_launch": t_a_minus * 1e6,
-                "gflops": 1872.0 * Vh * batch / t_a_minus / 1e9,
-                "other_kernels": {"ainv_hop": {"achieved": bytes_ainv * Vh * batch / t_ainv / 1e9, "us_per_launch": t_ainv * 1e6,
-                                               "frac": bytes_ainv * Vh * batch / t_ainv / 1e9 / peaks["hbm_gbs"],
-                                               "algorithmic_bytes_per_site_rhs": bytes_ainv}}}
-    if merged:   # the other fused variant of the iteration: s = r - alpha (A p - k^2 H tmp), same bytes, no reduction
-        t_s = kstats["ms_a_minus_hop_s"] / kstats["n_a_minus_hop_s"] * 1e-3
-        roofline["other_kernels"]["a_minus_hop_s"] = {"achieved": bytes_a_minus * Vh * batch / t_s / 1e9, "us_per_launch": t_s * 1e6,
-                                                      "frac": bytes_a_minus * Vh * batch / t_s / 1e9 / peaks["hbm_gbs"],
-                                                      "algorithmic_bytes_per_site_rhs": bytes_a_minus}
+        traffic_db = json.load(open(tp))
+
+    def entry(name):
+        kernel, n, ms_sum, bts, fl, tkey = table[name]
+        t = ms_sum / n * 1e-3
+        ach = bts * Vh * batch / t / 1e9
+        e = {"kernel": kernel, "achieved": ach, "frac": ach / peaks["hbm_gbs"], "us_per_launch": t * 1e6, "launches": n,
+             "algorithmic_bytes_per_site_rhs": bts, "algorithmic_bytes_per_launch": bts * Vh * batch,
+             "share_of_step": ms_sum / phases["ms_total"] if phases["ms_total"] else None,
+             "traffic": traffic_db.get(f"{tkey}_{cfg['name']}_b{batch}")}
+        if fl:
+            e["gflops"] = fl * Vh * batch / t / 1e9
+        return e
+    dominant = max(table, key=lambda k: table[k][2])
+    roofline = {"bound": "hbm", "name": dominant, "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_kind": peak_kind, "timed": timed,
+                "dominance": "largest summed device time of one kernel inside the timed steps (share_of_step = its launches' time / solve time)",
+                "traffic_source": traffic_db.get("source", "none: no ncu capture committed for this configuration")}
+    roofline.update(entry(dominant))
+    roofline["other_kernels"] = {k: entry(k) for k in table if k != dominant}
 
     # ---- the plain Wilson hop kernel timed alone (BASELINE.json: "clover Dslash GB/s"), fields larger than L2 or L2 flushed ----
     dslash = {}
@@ -388,11 +431,7 @@ def main():
                      "max_true_resid": max(i["true_resid"] for i in last["infos"]),
                      "phase_ms_per_step": {k: v / args.steps for k, v in phases.items()}}}
     if not args.no_cpu_baseline and world == 1:
-        run, n_it, cores = oracle_sample(cfg, 2, U)
-        v = run()
-        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                               "sample": f"2 oracle BiCGStab iterations of 1 source on {cfg['name']} (unpreconditioned fp64, OpenMP over sites), "
-                                         f"scaled to the {n_it} iterations the oracle needs for 1e-10 at these parameters on 8^3x16"}
+        out["cpu_baseline"] = oracle_full_solve(cfg, U)
     print(json.dumps(out))
     ctx.close()
 

@@ -53,7 +53,8 @@ typedef struct {
 
 typedef struct {
     int status;           /* 0 converged, 1 max_iter reached, 2 repeated breakdown (<r0,v> = 0 after 8 restarts), 3 non-finite */
-    int iters;            /* BiCGStab iterations of the batch this source was in */
+    int iters;            /* BiCGStab iterations of the BATCH this source was in (the rhs of a batch iterate together; a rhs that
+                             converges early is frozen, so every rhs of a batch reports the same count) */
     int reliable_updates; /* fp64 residual recomputations of that batch */
     double iter_resid;    /* the fp64 residual the convergence decision was taken on: ||b_e - Mhat y|| / ||eta|| of the last reliable
                              update, or the full-lattice residual when the final verification confirmed the claim itself */
@@ -167,6 +168,9 @@ typedef struct {
        n_a_minus_hop / ms_a_minus_hop count the one of Mhat s (with <t,s>, <t,t>, <r0,t>, <r0,s>) */
     long long n_a_minus_hop_s;
     double ms_a_minus_hop_s;
+    /* merged iteration: the one BLAS-1 sweep of the iteration (x, r, p updates with <q0,p>, ||r||^2: 9 vector passes) */
+    long long n_xrp_update;
+    double ms_xrp_update;
 } clover_solve_stats;
 int clover_get_stats(const clover_ctx *ctx, clover_solve_stats *out);
 

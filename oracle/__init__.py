@@ -63,6 +63,13 @@ def threads():
     return int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
 
 
+def set_threads(n):
+    """Set the OpenMP thread count of later oracle calls (bench.py reports a one-thread D-apply rate beside the all-cores one)."""
+    lib()
+    ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+    os.environ["OMP_NUM_THREADS"] = str(int(n))
+
+
 def hop(U, bc, psi):
     """(H psi)(x), SURVEY 8(c) O2."""
     U, psi = _c(U), _c(psi)

@@ -35,7 +35,7 @@ class SolveStats(ctypes.Structure):
                 ("ms_prep", ctypes.c_double), ("ms_iterate", ctypes.c_double), ("ms_reliable", ctypes.c_double),
                 ("ms_finish", ctypes.c_double), ("n_ainv_hop", ctypes.c_longlong), ("n_a_minus_hop", ctypes.c_longlong),
                 ("ms_ainv_hop", ctypes.c_double), ("ms_a_minus_hop", ctypes.c_double), ("n_a_minus_hop_s", ctypes.c_longlong),
-                ("ms_a_minus_hop_s", ctypes.c_double)]
+                ("ms_a_minus_hop_s", ctypes.c_double), ("n_xrp_update", ctypes.c_longlong), ("ms_xrp_update", ctypes.c_double)]
 
 
 _vp, _ip, _i, _d = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.c_int, ctypes.c_double

@@ -400,7 +400,9 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             q.r2 = q.maxr2 = d0;
             q.want_update = 0;
             if (!isfinite(d0)) { q.done = 1; q.status = 3; }
-            else if (d0 <= tol2 * q.eta2) { q.done = 1; q.beta = q.gam = q.alpha = st_z(zero); }
+            // freeze on a bound 1 % inside the tolerance: the status is decided later on the full-lattice residual (SC_FINAL), which
+            // equals this even-odd one only up to rounding, and a frozen rhs gets no further iteration
+            else if (d0 <= 0.98 * tol2 * q.eta2) { q.done = 1; q.beta = q.gam = q.alpha = st_z(zero); }
         }
         break;
     case SC_RESTART:  // after r0 := r: rho = <r0, r> = ||r||^2 (the value SC_RHO / SC_TRUE left in r2)

@@ -13,6 +13,10 @@ template <typename R> struct OpData {
     C *clov[2];       // A   : [parity], 36 complex per site (2 blocks x (3 packed diag pairs + 15 lower off-diag))
     C *clov_inv[2];   // A^-1, same packing
     int recon;        // 18 | 12
+    // Site-major ("packed") copies for the B = 8 kernels, fetched per CTA tile with one bulk async copy each (dslash3_kernel.cuh):
+    R *pk_link[2];     // [parity p of the OUTPUT site][cb][d = 2 mu + (fwd ? 0 : 1)][recon reals]: fwd = U_mu(x), bwd = U_mu(x - mu) as stored
+    R *pk_clov[2];     // [parity][cb][72 reals]: the 18 16-byte rows (fp32) of the packed blocks of A
+    R *pk_clov_inv[2]; // A^-1
 };
 
 // Per-rhs solver scalars, device resident (one entry per rhs of the batch).

@@ -72,51 +72,15 @@ __device__ __forceinline__ void hop_load2(const Geom &g, const OpData<float> &op
                                           HopIn2 &d)
 {
     bool wrap;
-    int nb = neighbour<MU, FWD>(g, cb, c, wrap);
-    // Ablation switches (experiments only, wrong results; profiles/r1_tuning.md "ablations"): which of the three parts of a
-    // direction -- neighbour gather, link load, arithmetic -- the kernel time is made of.
-#ifdef CLV_ABL_NB
-    nb = cb;   // all neighbours = own site: the gathers become L1 hits
-#endif
-#ifdef CLV_ABL_NOSPINOR
-#pragma unroll
-    for (int i = 0; i < 12; i++) {   // no gather at all: register data that the compiler cannot fold
-        d.psiA[i] = mk<float>(__int_as_float(0x3f800000 + cb + i), __int_as_float(0x3f900000 + rhs));
-        d.psiB[i] = mk<float>(__int_as_float(0x3fa00000 + cb - i), __int_as_float(0x3fb00000 + rhs));
-    }
-#else
+    const int nb = neighbour<MU, FWD>(g, cb, c, wrap);
     load_spinor2(in, (unsigned)nb * B + rhs, d.psiA, d.psiB);
-#endif
-#ifdef CLV_ABL_TGAUGE
-    if (MU == 3) { d.neg = wrap && g.bc[MU] < 0; return; }   // timing of a temporal-gauge hop: no t link at all
-#endif
-#ifdef CLV_ABL_NOLINK
-#pragma unroll
-    for (int i = 0; i < 9; i++) d.u[i] = mk<float>(__int_as_float(0x3f000000 + (cb >> 3) + i + 16 * MU), __int_as_float(0x3e800000 + i + FWD));
-#else
     if (FWD) load_link<RECON>(p ? op.gauge[1][MU] : op.gauge[0][MU], cb, d.u);
     else load_link<RECON>(p ? op.gauge[0][MU] : op.gauge[1][MU], nb, d.u);
-#endif
     d.neg = wrap && g.bc[MU] < 0;
 }
 
 template <int RECON, int MU, int FWD> __device__ __forceinline__ void hop_compute2(HopIn2 &d, HopAcc<float> &accA, HopAcc<float> &accB)
 {
-#ifdef CLV_ABL_NOCOMPUTE
-    {   // loads only: every loaded word is consumed by one add
-        float sA = 0.f, sB = 0.f, su = 0.f;
-#pragma unroll
-        for (int i = 0; i < 12; i++) {
-            sA += d.psiA[i].re + d.psiA[i].im;
-            sB += d.psiB[i].re + d.psiB[i].im;
-        }
-#pragma unroll
-        for (int i = 0; i < RECON / 2; i++) su += d.u[i].re + d.u[i].im;
-        accA.ure[MU % 3].x += sA + su;
-        accB.ure[MU % 3].x += sB + su;
-        return;
-    }
-#endif
     cx<float> hA[6], hB[6];
     third_row<float, RECON>(d.u);
     project<float, MU, FWD>(d.psiA, hA);
@@ -128,13 +92,6 @@ template <int RECON, int MU, int FWD> __device__ __forceinline__ void hop_comput
             hB[i] = mk<float>(-hB[i].re, -hB[i].im);
         }
     }
-#ifdef CLV_ABL_TGAUGE
-    if (MU == 3) {
-        accA.template add_unit_t<FWD>(hA);
-        accB.template add_unit_t<FWD>(hB);
-        return;
-    }
-#endif
     accA.template add<MU, FWD>(hA, d.u);
     accB.template add<MU, FWD>(hB, d.u);
 }

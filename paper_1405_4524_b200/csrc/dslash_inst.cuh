@@ -1,7 +1,8 @@
 // dslash_inst.cuh -- host dispatch of one (precision, batch) family of Dslash kernels; included by the
 // dslash_<prec>_b<B>.cu instantiation units so the variants compile in parallel.
 #pragma once
-#include "dslash2_kernel.cuh"
+#include "dslash3_kernel.cuh"
+#include <algorithm>
 #include <cstdlib>
 
 namespace clv {
@@ -42,6 +43,45 @@ static int launch_dslash2_BR(const clover_ctx *ctx, const OpData<float> &op, con
     CLV_CUDA(cudaGetLastError());
     return 0;
 }
+// fp32, B = 8: the persistent kernel of dslash3_kernel.cuh (operator data by bulk async copy); grid = resident CTAs of the device
+template <int B, int RECON>
+static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
+{
+    const Geom &g = ctx->geom;
+    static const int n_sm = [] { int dev = 0, n = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); return n; }();
+    const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
+#define CLV_LAUNCH3(XM, PI, DT)                                                                                          \
+    case (XM) * 100 + (PI) * 10 + (DT): {                                                                                \
+        constexpr int BLK = CLV_HAS_RED(DT) ? CLV_R2_BLOCK_DOT : CLV_R2_BLOCK_NODOT;                                     \
+        auto kern = dslash3_kernel<B, RECON, XM, PI, DT, BLK>;                                                           \
+        static const cudaError_t attr = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
+        CLV_CUDA(attr);                                                                                                  \
+        const unsigned ntiles = ((unsigned)g.Vh + (2 * BLK / B) - 1) / (2 * BLK / B);                                    \
+        const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * (CLV_R3_CTAS_PER_SM_WARPS * 32 / BLK));        \
+        if (grid_out) *grid_out = (int)grid;                                                                             \
+        kern<<<grid, BLK, 0, st>>>(g, op, a);                                                                            \
+        break;                                                                                                           \
+    }
+    switch (key) {
+        CLV_LAUNCH3(XM_NONE, 0, DOT_NONE)
+        CLV_LAUNCH3(XM_NONE, 1, DOT_NONE)
+        CLV_LAUNCH3(XM_PLAIN, 0, DOT_NONE)
+        CLV_LAUNCH3(XM_PLAIN, 1, DOT_NONE)
+        CLV_LAUNCH3(XM_CLOVER, 0, DOT_NONE)
+        CLV_LAUNCH3(XM_CLOVER, 0, DOT_W)
+        CLV_LAUNCH3(XM_CLOVER, 0, DOT_X)
+        CLV_LAUNCH3(XM_CLOVER, 0, DOT_RES)
+        CLV_LAUNCH3(XM_CLOVER, 0, DOT_S)
+        CLV_LAUNCH3(XM_CLOVER, 0, DOT_XW)
+    default:
+        set_error("dslash: unsupported variant xmode=%d pinv=%d dot=%d", a.xmode, a.pinv, a.dot);
+        return CLOVER_EINVAL;
+    }
+#undef CLV_LAUNCH3
+    CLV_CUDA(cudaGetLastError());
+    return 0;
+}
+
 template <typename R, int B, int RECON> struct PairLaunch {   // double, or B = 1: no pair kernel
     static bool use() { return false; }
     static int go(const clover_ctx *, const OpData<R> &, const DslashArgs<R> &, cudaStream_t, int *) { return CLOVER_EINVAL; }
@@ -59,7 +99,13 @@ template <int B, int RECON> struct PairLaunchF {
 };
 template <int RECON> struct PairLaunch<float, 2, RECON> : PairLaunchF<2, RECON> {};
 template <int RECON> struct PairLaunch<float, 4, RECON> : PairLaunchF<4, RECON> {};
-template <int RECON> struct PairLaunch<float, 8, RECON> : PairLaunchF<8, RECON> {};
+template <int RECON> struct PairLaunch<float, 8, RECON> : PairLaunchF<8, RECON> {
+    static int go(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
+    {
+        static const bool r3 = [] { const char *e = getenv("CLOVER_R3"); return e ? atoi(e) != 0 : false; }();  // tuning/debug knob only
+        return r3 ? launch_dslash3_BR<8, RECON>(ctx, op, a, st, grid_out) : launch_dslash2_BR<8, RECON>(ctx, op, a, st, grid_out);
+    }
+};
 
 
 template <typename R, int B, int RECON>

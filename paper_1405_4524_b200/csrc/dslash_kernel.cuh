@@ -160,19 +160,6 @@ template <> struct HopAcc<float> {
             }
         }
     }
-    // mu = t with a unit link (temporal gauge): g = h, no SU(3) product
-    template <int FWD> __device__ __forceinline__ void add_unit_t(const cx<float> h[6])
-    {
-        constexpr float s = FWD ? -1.f : 1.f;
-#pragma unroll
-        for (int a = 0; a < 3; a++) {
-            const float2 gre = make_float2(h[a].re, h[3 + a].re), gim = make_float2(h[a].im, h[3 + a].im);
-            ure[a] = __fadd2_rn(ure[a], gre);
-            uim[a] = __fadd2_rn(uim[a], gim);
-            lre[a] = __ffma2_rn(gre, make_float2(s, s), lre[a]);
-            lim[a] = __ffma2_rn(gim, make_float2(s, s), lim[a]);
-        }
-    }
     __device__ __forceinline__ void finish(cx<float> out[12]) const
     {
 #pragma unroll
@@ -197,10 +184,7 @@ __device__ __forceinline__ void hop_load(const Geom &g, const OpData<R> &op, con
                                          const Coord &c, HopIn<R> &d)
 {
     bool wrap;
-    int nb = neighbour<MU, FWD>(g, cb, c, wrap);
-#ifdef CLV_FAKE_NB
-    nb = cb;  // experiment only: all neighbours = own site (upper bound of L1 reuse)
-#endif
+    const int nb = neighbour<MU, FWD>(g, cb, c, wrap);
     load_spinor(in, (unsigned)nb * B + rhs, d.psi);
     // (ternaries rather than op.gauge[p]: runtime indexing of a kernel parameter would force a local copy)
     if (FWD) load_link<RECON>(p ? op.gauge[1][MU] : op.gauge[0][MU], cb, d.u);

@@ -54,6 +54,33 @@ __global__ void reorder_gauge_kernel(Geom g, const double *__restrict__ gauge, O
     for (int k = 0; k < RECON32 / 2; k++) o32.gauge[p][mu][cplx_index<float>(cb, k, RECON32 / 2)] = make_float2((float)u[k].re, (float)u[k].im);
 }
 
+// Site-major fp32 copies for the B = 8 kernels: per output site of parity p the 8 links of its hop, in the order d = 2 mu + (fwd ? 0 : 1)
+// (fwd: U_mu(x); bwd: U_mu(x - mu), stored as it is and daggered in-kernel), rounded to fp32 exactly as the lane-blocked copy is.
+template <int RECON32> __global__ void pack_links_kernel(Geom g, const double *__restrict__ gauge, OpData<float> o32)
+{
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= g.Vh) return;
+    const int p = blockIdx.y >> 3, d = blockIdx.y & 7, mu = d >> 1;
+    const long V = 2L * g.Vh;
+    const Lex x = lex_of(g, cb, p);
+    zc u[9];
+    ld_link(gauge, V, mu, lex_index(g, (d & 1) ? shifted(g, x, mu, -1) : x), u);
+    float2 *o = reinterpret_cast<float2 *>(o32.pk_link[p] + ((size_t)cb * 8 + d) * RECON32);
+#pragma unroll
+    for (int k = 0; k < RECON32 / 2; k++) o[k] = make_float2((float)u[k].re, (float)u[k].im);
+}
+// lane-blocked rows of the packed clover blocks -> 18 consecutive 16-byte rows per site
+__global__ void pack_clover_kernel(Geom g, OpData<float> o32)
+{
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (unsigned)g.Vh * 18u) return;
+    const unsigned cb = i / 18u, row = i % 18u;
+    const int p = blockIdx.y >> 1;
+    const float2 *src = (blockIdx.y & 1) ? o32.clov_inv[p] : o32.clov[p];
+    float *dst = (blockIdx.y & 1) ? o32.pk_clov_inv[p] : o32.pk_clov[p];
+    reinterpret_cast<float4 *>(dst)[i] = __ldg(reinterpret_cast<const float4 *>(src) + ((size_t)(cb >> 5) * 18 + row) * 32 + (cb & 31u));
+}
+
 // ---- S1: clover term ------------------------------------------------------------------------------
 __device__ __forceinline__ void mm(const zc a[9], const zc b[9], zc c[9])  // c = a b
 {
@@ -327,12 +354,12 @@ template int reorder_out<double, double>(const Geom &, double *, const double2 *
 template int reorder_out<float, float>(const Geom &, float *, const float4 *, const float4 *, int, cudaStream_t);
 
 // ---- clover_create's device work ---------------------------------------------------------------
-template <typename T> static int dev_alloc(clover_ctx *ctx, T **p, size_t count)
+template <typename T> static int dev_alloc(clover_ctx *ctx, T **p, size_t count, cudaStream_t st)
 {
     void *q = nullptr;
     CLV_CUDA(cudaMalloc(&q, count * sizeof(T)));
     ctx->allocs.push_back(q);
-    CLV_CUDA(cudaMemset(q, 0, count * sizeof(T)));
+    CLV_CUDA(cudaMemsetAsync(q, 0, count * sizeof(T), st));   // padding lanes must read as zeros; ordered before the fill kernels on `st`
     *p = (T *)q;
     return 0;
 }
@@ -343,23 +370,34 @@ int setup_operator(clover_ctx *ctx, const double *gauge_dev, cudaStream_t st)
     const size_t nb = lb_blocks(g.Vh) * 32u;  // padded entries per parity
     for (int p = 0; p < 2; p++) {
         for (int mu = 0; mu < 4; mu++) {
-            CLV_CHECK(dev_alloc(ctx, &ctx->op64.gauge[p][mu], nb * 9));
-            CLV_CHECK(dev_alloc(ctx, &ctx->op32.gauge[p][mu], nb * (ctx->op32.recon / 2)));
+            CLV_CHECK(dev_alloc(ctx, &ctx->op64.gauge[p][mu], nb * 9, st));
+            CLV_CHECK(dev_alloc(ctx, &ctx->op32.gauge[p][mu], nb * (ctx->op32.recon / 2), st));
         }
-        CLV_CHECK(dev_alloc(ctx, &ctx->op64.clov[p], nb * 36));
-        CLV_CHECK(dev_alloc(ctx, &ctx->op64.clov_inv[p], nb * 36));
-        CLV_CHECK(dev_alloc(ctx, &ctx->op32.clov[p], nb * 36));
-        CLV_CHECK(dev_alloc(ctx, &ctx->op32.clov_inv[p], nb * 36));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op64.clov[p], nb * 36, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op64.clov_inv[p], nb * 36, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.clov[p], nb * 36, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.clov_inv[p], nb * 36, st));
+    }
+    for (int p = 0; p < 2; p++) {
+        ctx->op64.pk_link[p] = ctx->op64.pk_clov[p] = ctx->op64.pk_clov_inv[p] = nullptr;   // fp32 only
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_link[p], (size_t)g.Vh * 8 * ctx->op32.recon, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov[p], (size_t)g.Vh * 72, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov_inv[p], (size_t)g.Vh * 72, st));
     }
     int *singular = nullptr;
-    CLV_CHECK(dev_alloc(ctx, &singular, 1));
-    CLV_CUDA(cudaStreamSynchronize(0));  // the memsets above ran on the legacy stream
+    CLV_CHECK(dev_alloc(ctx, &singular, 1, st));
     dim3 gg((g.Vh + 127) / 128, 8);
     if (ctx->op32.recon == 12) reorder_gauge_kernel<12><<<gg, 128, 0, st>>>(g, gauge_dev, ctx->op64, ctx->op32);
     else reorder_gauge_kernel<18><<<gg, 128, 0, st>>>(g, gauge_dev, ctx->op64, ctx->op32);
     CLV_CUDA(cudaGetLastError());
     dim3 gc((g.Vh + 63) / 64, 2);
     clover_build_kernel<<<gc, 64, 0, st>>>(g, gauge_dev, ctx->csw * ctx->kappa, ctx->op64, ctx->op32, singular);
+    CLV_CUDA(cudaGetLastError());
+    dim3 gp((g.Vh + 127) / 128, 16);
+    if (ctx->op32.recon == 12) pack_links_kernel<12><<<gp, 128, 0, st>>>(g, gauge_dev, ctx->op32);
+    else pack_links_kernel<18><<<gp, 128, 0, st>>>(g, gauge_dev, ctx->op32);
+    CLV_CUDA(cudaGetLastError());
+    pack_clover_kernel<<<dim3(((unsigned)g.Vh * 18u + 255u) / 256u, 4), 256, 0, st>>>(g, ctx->op32);
     CLV_CUDA(cudaGetLastError());
     int h = 0;
     CLV_CUDA(cudaMemcpyAsync(&h, singular, sizeof(int), cudaMemcpyDeviceToHost, st));

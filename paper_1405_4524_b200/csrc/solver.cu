@@ -74,7 +74,9 @@ void free_work(clover_ctx *ctx)
     ctx->work = nullptr;
 }
 
-static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
+// Workspaces are (re)allocated only when a call needs more than the context holds; their one-time clears are queued on the
+// caller's stream, so a call that finds everything in place touches no other stream and never synchronises the device.
+static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging, cudaStream_t st)
 {
     if (!ctx->work) ctx->work = new SolveWork();
     SolveWork *W = ctx->work;
@@ -85,24 +87,24 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
             cudaFree(W->f64[i]);
             W->f64[i] = nullptr;
             CLV_CUDA(cudaMalloc(&W->f64[i], n64 * sizeof(double2)));
-            CLV_CUDA(cudaMemset(W->f64[i], 0, n64 * sizeof(double2)));
+            CLV_CUDA(cudaMemsetAsync(W->f64[i], 0, n64 * sizeof(double2), st));
         }
         cudaFree(W->partial);
         // twice the blocks of one Dslash launch: the final verification reduces the partials of two launches (even + odd) at once
         W->partial_blocks = 2 * std::max<int>(((unsigned)g.Vh * B + dslash_block_size() - 1) / dslash_block_size(), 148 * 8);
         CLV_CUDA(cudaMalloc(&W->partial, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
-        CLV_CUDA(cudaMemset(W->partial, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
+        CLV_CUDA(cudaMemsetAsync(W->partial, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double), st));
         cudaFree(W->partial2);
         CLV_CUDA(cudaMalloc(&W->partial2, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
-        CLV_CUDA(cudaMemset(W->partial2, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
+        CLV_CUDA(cudaMemsetAsync(W->partial2, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double), st));
         if (!W->sc_dev) {
             CLV_CUDA(cudaMalloc(&W->sc_dev, 8 * sizeof(RhsScalars)));
-            CLV_CUDA(cudaMemset(W->sc_dev, 0, 8 * sizeof(RhsScalars)));
+            CLV_CUDA(cudaMemsetAsync(W->sc_dev, 0, 8 * sizeof(RhsScalars), st));
             CLV_CUDA(cudaHostAlloc((void **)&W->sc_host, 8 * sizeof(RhsScalars), cudaHostAllocMapped));
             CLV_CUDA(cudaHostGetDevicePointer((void **)&W->sc_host_dev, W->sc_host, 0));
             CLV_CUDA(cudaMalloc(&W->stage, 8 * 32 * 8 * sizeof(double)));
             CLV_CUDA(cudaMalloc(&W->ticket, 8 * sizeof(unsigned)));
-            CLV_CUDA(cudaMemset(W->ticket, 0, 8 * sizeof(unsigned)));
+            CLV_CUDA(cudaMemsetAsync(W->ticket, 0, 8 * sizeof(unsigned), st));
         }
         W->B_cap = B;
         W->sloppy_bytes = 0;
@@ -114,7 +116,7 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
             cudaFree(W->sl[i]);
             W->sl[i] = nullptr;
             CLV_CUDA(cudaMalloc(&W->sl[i], need));
-            CLV_CUDA(cudaMemset(W->sl[i], 0, need));
+            CLV_CUDA(cudaMemsetAsync(W->sl[i], 0, need, st));
         }
         W->sloppy_bytes = need;
         if (W->iter_graph) { cudaGraphExecDestroy(W->iter_graph); W->iter_graph = nullptr; }
@@ -148,7 +150,6 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging)
         CLV_CUDA(cudaEventCreateWithFlags(&W->ev_dep, cudaEventDisableTiming));
         W->have_ev = true;
     }
-    CLV_CUDA(cudaDeviceSynchronize());  // the memsets above ran on the legacy stream
     return 0;
 }
 
@@ -409,7 +410,9 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
         CLV_CUDA(cudaEventRecord(W->kev[5], st));
         nl += 3;
         CLV_CHECK(blas_scalar_step(bc, SC_OMEGA2, grid, tol2, delta2));
+        CLV_CUDA(cudaEventRecord(W->kev[0], st));
         CLV_CHECK(blas_xrp_update<R>(bc, x, r, p, s, t, q0, &nb));
+        CLV_CUDA(cudaEventRecord(W->kev[3], st));
         CLV_CHECK(blas_scalar_step(bc, SC_RHO2, nb, tol2, delta2, W->sc_host_dev));
         CLV_CUDA(cudaEventRecord(W->ev_flags, st));
         return 0;
@@ -427,7 +430,8 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
             CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[2], W->kev[4])); S.ms_ainv_hop += ms;
             CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[1], W->kev[2])); S.ms_a_minus_hop_s += ms;
             CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[4], W->kev[5])); S.ms_a_minus_hop += ms;
-            S.n_ainv_hop += 2; S.n_a_minus_hop_s++; S.n_a_minus_hop++;
+            CLV_CUDA(cudaEventElapsedTime(&ms, W->kev[0], W->kev[3])); S.ms_xrp_update += ms;
+            S.n_ainv_hop += 2; S.n_a_minus_hop_s++; S.n_a_minus_hop++; S.n_xrp_update++;
         } else if (use_graph && need_p) {
             CLV_CUDA(cudaGraphLaunch(W->iter_graph, st));
             nl += W->graph_kernels;
@@ -529,7 +533,7 @@ static int next_batch(int remaining, int batch)
 int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, double tol, int max_iter, int batch, int mixed, clover_rhs_info *info,
                   cudaStream_t st, int host_buffers)
 {
-    CLV_CHECK(ensure_work(ctx, batch, mixed ? 4 : 8, host_buffers != 0));
+    CLV_CHECK(ensure_work(ctx, batch, mixed ? 4 : 8, host_buffers != 0, st));
     SolveWork *W = ctx->work;
     memset(&ctx->stats, 0, sizeof ctx->stats);
     const size_t per_rhs = (size_t)2 * ctx->geom.Vh * 24;  // doubles per canonical spinor
@@ -553,25 +557,37 @@ int solve_batches(clover_ctx *ctx, const double *src, double *dst, int n_rhs, do
     int nb = 0, start[64], size[64];
     for (int done = 0; done < n_rhs && nb < 64; done += size[nb - 1]) { start[nb] = done; size[nb] = next_batch(n_rhs - done, batch); nb++; }
     if (nb == 64 && start[63] + size[63] < n_rhs) { set_error("clover_solve_host: more than 64 batches in one call"); return CLOVER_EINVAL; }
-    auto h2d = [&](int i) {
-        return cudaMemcpyAsync(W->stage_in[i & 1], src + start[i] * per_rhs, per_rhs * size[i] * sizeof(double), cudaMemcpyHostToDevice, W->s_in) ||
-               cudaEventRecord(W->ev_in[i & 1], W->s_in);
+    auto h2d = [&](int i) -> cudaError_t {
+        const cudaError_t e = cudaMemcpyAsync(W->stage_in[i & 1], src + start[i] * per_rhs, per_rhs * size[i] * sizeof(double), cudaMemcpyHostToDevice, W->s_in);
+        return e != cudaSuccess ? e : cudaEventRecord(W->ev_in[i & 1], W->s_in);
     };
-    CLV_CUDA((cudaError_t)h2d(0));
+    // an error return must not leave copies in flight that read or write the caller's host buffers
+    auto drain = [&]() { cudaStreamSynchronize(W->s_in); cudaStreamSynchronize(W->s_out); };
+#define CLV_CUDA_DRAIN(call)                                                                                    \
+    do {                                                                                                        \
+        const cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess) {                                                                                \
+            drain();                                                                                            \
+            set_error("%s failed at %s:%d: %s", #call, __FILE__, __LINE__, cudaGetErrorString(e_));             \
+            return (e_ == cudaErrorMemoryAllocation) ? CLOVER_ENOMEM : CLOVER_ECUDA;                            \
+        }                                                                                                       \
+    } while (0)
+    CLV_CUDA_DRAIN(h2d(0));
     for (int i = 0; i < nb; i++) {
         const int B = size[i], k = i & 1;
-        if (i + 1 < nb) CLV_CUDA((cudaError_t)h2d(i + 1));
-        if (B != lastB) CLV_CHECK(clear_fields(W, ctx->geom, B, st));
+        if (i + 1 < nb) CLV_CUDA_DRAIN(h2d(i + 1));
+        if (B != lastB) { const int rc = clear_fields(W, ctx->geom, B, st); if (rc < 0) { drain(); return rc; } }
         lastB = B;
-        CLV_CUDA(cudaStreamWaitEvent(st, W->ev_in[k], 0));
-        if (i >= 2) CLV_CUDA(cudaStreamWaitEvent(st, W->ev_out[k], 0));  // D2H of batch i-2 has drained stage_out[k]
+        CLV_CUDA_DRAIN(cudaStreamWaitEvent(st, W->ev_in[k], 0));
+        if (i >= 2) CLV_CUDA_DRAIN(cudaStreamWaitEvent(st, W->ev_out[k], 0));  // D2H of batch i-2 has drained stage_out[k]
         int rc = mixed ? solve_batch<float>(ctx, W->stage_in[k], W->stage_out[k], B, tol, max_iter, info + start[i], st)
                        : solve_batch<double>(ctx, W->stage_in[k], W->stage_out[k], B, tol, max_iter, info + start[i], st);
-        if (rc < 0) return rc;
+        if (rc < 0) { drain(); return rc; }
         bad += rc;
-        CLV_CUDA(cudaMemcpyAsync(dst + start[i] * per_rhs, W->stage_out[k], per_rhs * B * sizeof(double), cudaMemcpyDeviceToHost, W->s_out));
-        CLV_CUDA(cudaEventRecord(W->ev_out[k], W->s_out));
+        CLV_CUDA_DRAIN(cudaMemcpyAsync(dst + start[i] * per_rhs, W->stage_out[k], per_rhs * B * sizeof(double), cudaMemcpyDeviceToHost, W->s_out));
+        CLV_CUDA_DRAIN(cudaEventRecord(W->ev_out[k], W->s_out));
     }
+#undef CLV_CUDA_DRAIN
     CLV_CUDA(cudaStreamSynchronize(W->s_out));
     return bad;
 }
@@ -635,7 +651,7 @@ template <typename R> static int apply_chunk(clover_ctx *ctx, int op, const R *i
 
 int apply_op(clover_ctx *ctx, int op, int precision, const void *in, void *out, int n_rhs, cudaStream_t st)
 {
-    CLV_CHECK(ensure_work(ctx, std::min(8, ctx->max_rhs), 4, false));
+    CLV_CHECK(ensure_work(ctx, std::min(8, ctx->max_rhs), 4, false, st));
     const size_t per_rhs = (size_t)2 * ctx->geom.Vh * 24;
     int lastB = -1;
     for (int done = 0; done < n_rhs;) {
@@ -706,7 +722,7 @@ template <typename R> static int bench_impl(clover_ctx *ctx, int kernel, int B, 
 
 int bench_kernel(clover_ctx *ctx, int kernel, int precision, int n_rhs, int reps, int flush_l2, float *ms, cudaStream_t st)
 {
-    CLV_CHECK(ensure_work(ctx, n_rhs, 4, false));
+    CLV_CHECK(ensure_work(ctx, n_rhs, 4, false, st));
     return precision == 32 ? bench_impl<float>(ctx, kernel, n_rhs, reps, flush_l2, ms, st) : bench_impl<double>(ctx, kernel, n_rhs, reps, flush_l2, ms, st);
 }
 

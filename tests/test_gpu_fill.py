@@ -54,3 +54,27 @@ def test_fill_of_solved_noise_approaches_the_propagator():
     expected = np.sqrt((12 * 64 * 8 - 1) / n)
     assert 0.5 < rel / expected < 2.0
     ctx.close()
+
+
+def test_fill_at_the_bench_size_sampled_blocks():
+    """8^3x16, N_r = 32 (the paper's Table II size, the size bench.py times; 9.66 GB per array): 192 x 192 blocks (three 64 x 64
+    CTA tiles each way: 16 sites x 12 spin-colour rows, 16 sites x 12 columns) of S and of S^dagger against oracle/fill.py run on
+    the same slices of the inputs -- first, interior and last tiles of the grid, t0 = 5."""
+    from paper_1405_4524_b200 import binding as B
+    dims, n, t0 = (8, 8, 8, 16), 32, 5
+    X = wl.random_spinor(dims, 31, n)
+    eta = wl.random_spinor(dims, 32, n)
+    xd, ed = torch.from_numpy(X).cuda(), torch.from_numpy(eta).cuda()
+    V3, T = 512, 16
+    Xf, ef = X.reshape(n, T, V3, 12), eta.reshape(n, T, V3, 12)
+    blocks = [(0, 0, 0), (7, 200, 304), (T - 1, V3 - 16, V3 - 16), (T - 1, 0, V3 - 16), (3, V3 - 16, 0)]   # (t, first z3, first x3)
+    for dagger in (False, True):
+        S = B.stochastic_fill(xd, ed, t0=t0, scale=wl.INV_SQRT2, dagger=dagger)
+        for t, z0, x0 in blocks:
+            xs = Xf[:, t, z0:z0 + 16].reshape(n, 1, 1, 1, 16, 4, 3)
+            es = ef[:, t0, x0:x0 + 16].reshape(n, 1, 1, 1, 16, 4, 3)
+            want = fill.stochastic_fill(xs, es, t0=0, scale=wl.INV_SQRT2, dagger=dagger)
+            got = (S[x0:x0 + 16, :, t, z0:z0 + 16] if dagger else S[t, z0:z0 + 16, :, x0:x0 + 16]).cpu().numpy()
+            want = want[:, :, 0] if dagger else want[0]
+            assert got.shape == want.shape and nerr(got, want) < 1e-13, (dagger, t, z0, x0)
+        del S

@@ -1,8 +1,13 @@
-"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (cfg 3: 24^3x48, batch 8, mixed;
-cfg 4: 32^3x64, two-row links, time dilution).  The oracle cannot solve these in seconds, so: (a) the fused operators are
-compared element by element on whole fields (one oracle D apply ~ 1 s), (b) every checked GPU solution gets an
-oracle-computed true residual, (c) solution parity is checked through the property psi = D^-1 eta <=> D psi = eta with the
-oracle's D, which pins psi to the unique solution within cond(D) * 1e-10."""
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (cfg 2: 16^3x32, batch 4, mixed, the
+iteration replayed as a CUDA graph; cfg 3: 24^3x48, batch 8, mixed; cfg 4: 32^3x64, two-row links, time dilution).
+
+What is compared (BASELINE.json north_star: "match the CPU oracle within the stated tolerances on every config ... solutions
+within 1e-8 relative at a true fp64 residual <= 1e-10"; the system solved is D X = eta):
+  (a) the fused operators element by element on whole fields, fp64 1e-13 and fp32 1e-6 (scale-normalised, R9);
+  (b) EVERY solved source gets its true residual ||eta - D psi|| / ||eta|| recomputed with the ORACLE's D, which must meet the
+      tolerance and agree with the residual the library reports;
+  (c) oracle-solved sources (the oracle's own unpreconditioned fp64 BiCGStab to 1e-12, tens of seconds each at these sizes):
+      ||psi - psi_oracle|| / ||psi_oracle|| < 1e-8 in the 2-norm and max-normalised."""
 import numpy as np
 import pytest
 import torch
@@ -12,44 +17,85 @@ from paper_1405_4524_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
+SOL_TOL = 1e-8       # north_star: solutions within 1e-8 relative
+ORACLE_TOL = 1e-12   # the oracle's own stopping tolerance for the solutions it is compared on
 
-def _run(ci, n_solve, check):
-    from paper_1405_4524_b200 import binding as B
-    c = wl.CONFIGS[ci]
-    dims = c["dims"]
-    U = wl.gauge_links(dims, c["eps"], c["gauge_seed"])
-    A = oracle.clover_matrix(U, c["kappa"], c["csw"])
-    ctx = B.Clover(torch.from_numpy(U).cuda(), c["kappa"], c["csw"], bc=wl.BC, recon=c["recon"], max_rhs=8)
-    # sources of the first and the last batch of the config (cfg 4: timeslices 0.. and ..63)
-    first = B.noise_fill(dims, c["noise_seed"], n_solve, rhs_offset=0, time_dilution=c["dilution"], scale=wl.INV_SQRT2)
-    last = B.noise_fill(dims, c["noise_seed"], n_solve, rhs_offset=c["n_rhs"] - n_solve, time_dilution=c["dilution"], scale=wl.INV_SQRT2)
-    want = oracle.noise_fill(dims, c["noise_seed"], 1, rhs_offset=c["n_rhs"] - 1, time_dilution=c["dilution"], scale=wl.INV_SQRT2)
-    assert np.array_equal(last[-1].cpu().numpy().view(np.uint64), want[0].view(np.uint64))        # noise bit-exact at full size
-    # operators on whole fields, fp64 and fp32 (the batch-8 kernels)
-    x = first.cpu().numpy()
-    ref = oracle.apply_D(U, A, wl.BC, c["kappa"], x[0])
+
+def _oracle_residual(U, A, kappa, eta, psi):
+    return np.linalg.norm(eta - oracle.apply_D(U, A, wl.BC, kappa, psi)) / np.linalg.norm(eta)
+
+
+def _check_solution(U, A, kappa, eta, psi):
+    want, oi = oracle.bicgstab(U, A, wl.BC, kappa, eta, tol=ORACLE_TOL)
+    assert oi["status"] == 0 and oi["true_resid"] < 10 * ORACLE_TOL, oi
+    d = psi - want
+    l2 = np.linalg.norm(d) / np.linalg.norm(want)
+    mx = np.abs(d).max() / np.abs(want).max()
+    assert l2 < SOL_TOL and mx < SOL_TOL, (l2, mx, oi)
+    return l2, mx
+
+
+def _operators(ctx, B, U, A, c, first):
+    """(a): D and H on whole fields through the batched kernels, fp64 and fp32."""
+    x = first[0].cpu().numpy()
+    ref = oracle.apply_D(U, A, wl.BC, c["kappa"], x)
     got = ctx.dslash_apply(B.OP_D_FULL, first)[0].cpu().numpy()
     assert np.abs(got - ref).max() / np.abs(ref).max() < 1e-13
     got32 = ctx.dslash_apply(B.OP_D_FULL, first.to(torch.complex64))[0].cpu().numpy()
     assert np.abs(got32 - ref).max() / np.abs(ref).max() < 1e-6
-    hop = oracle.hop(U, wl.BC, x[0])
+    hop = oracle.hop(U, wl.BC, x)
     got32 = ctx.dslash_apply(B.OP_HOP_FULL, first.to(torch.complex64))[0].cpu().numpy()
     assert np.abs(got32 - hop).max() / np.abs(hop).max() < 1e-6
-    del got, got32, ref, hop
-    for eta in (first, last):
+
+
+def _run(ci, chunks, oracle_solved):
+    """chunks: list of (rhs_offset, count) noise windows of the config, each solved in the config's batch size;
+    oracle_solved: global source numbers that are also solved by the oracle and compared."""
+    from paper_1405_4524_b200 import binding as B
+    c = wl.CONFIGS[ci]
+    dims, kappa = c["dims"], c["kappa"]
+    U = wl.gauge_links(dims, c["eps"], c["gauge_seed"])
+    A = oracle.clover_matrix(U, kappa, c["csw"])
+    ctx = B.Clover(torch.from_numpy(U).cuda(), kappa, c["csw"], bc=wl.BC, recon=c["recon"], max_rhs=8)
+    want = oracle.noise_fill(dims, c["noise_seed"], 1, rhs_offset=c["n_rhs"] - 1, time_dilution=c["dilution"], scale=wl.INV_SQRT2)
+    got = B.noise_fill(dims, c["noise_seed"], 1, rhs_offset=c["n_rhs"] - 1, time_dilution=c["dilution"], scale=wl.INV_SQRT2)
+    assert np.array_equal(got[0].cpu().numpy().view(np.uint64), want[0].view(np.uint64))        # noise bit-exact at full size
+    del want, got
+    seen = set()
+    for k, (off, cnt) in enumerate(chunks):
+        eta = B.noise_fill(dims, c["noise_seed"], cnt, rhs_offset=off, time_dilution=c["dilution"], scale=wl.INV_SQRT2)
+        if k == 0:
+            _operators(ctx, B, U, A, c, eta[: c["batch"]].contiguous())
         psi, infos, bad = ctx.solve(eta, tol=wl.TOL, batch=c["batch"], mixed=bool(c["mixed"]))
         assert bad == 0, infos
         e, p = eta.cpu().numpy(), psi.cpu().numpy()
-        for r in check:
-            res = np.linalg.norm(e[r] - oracle.apply_D(U, A, wl.BC, c["kappa"], p[r])) / np.linalg.norm(e[r])
-            assert res <= wl.TOL, (r, res)
-            assert abs(infos[r]["true_resid"] - res) <= 1e-3 * res + 1e-14
+        del eta, psi
+        for r in range(cnt):
+            res = _oracle_residual(U, A, kappa, e[r], p[r])                                     # (b), every solved source
+            assert res <= wl.TOL, (off + r, res)
+            assert abs(infos[r]["true_resid"] - res) <= 1e-3 * res + 1e-14, (off + r, res, infos[r])
+            if off + r in oracle_solved:
+                if c["dilution"]:   # time dilution: source off + r lives on timeslice (off + r) mod T only
+                    t_r = (off + r) % dims[3]
+                    assert np.count_nonzero(e[r][t_r]) == e[r][t_r].size and np.count_nonzero(e[r]) == e[r][t_r].size
+                _check_solution(U, A, kappa, e[r], p[r])                                        # (c)
+                seen.add(off + r)
+    assert seen == set(oracle_solved)
     ctx.close()
 
 
+def test_cfg2_16x16x16x32_batch4_mixed_graph():
+    # all 16 sources in 4 batches of 4 (the graph-replayed mixed-precision iteration); oracle solves: first of the first batch,
+    # last of the last batch
+    _run(2, [(0, 16)], oracle_solved=(0, 15))
+
+
 def test_cfg3_24x24x24x48_batch8_mixed():
-    _run(3, 8, check=(0, 7))
+    # all 32 sources of the headline configuration, as bench.py solves them; one oracle-solved source
+    _run(3, [(0, 16), (16, 16)], oracle_solved=(0,))
 
 
 def test_cfg4_32x32x32x64_recon12_dilution():
-    _run(4, 8, check=(7,))
+    # first and last batch of the 64 time-diluted sources (timeslices 0..7 and 56..63); oracle solves: source 0 and the source on
+    # timeslice 63
+    _run(4, [(0, 8), (56, 8)], oracle_solved=(0, 63))

@@ -250,3 +250,30 @@ def test_merged_and_textbook_iteration_agree(B, mixed, monkeypatch):
         assert np.linalg.norm(out["1"][0][r] - out["0"][0][r]) / np.linalg.norm(out["0"][0][r]) < 2e-9
         assert abs(out["1"][1][r]["iters"] - out["0"][1][r]["iters"]) <= 4
     S.ctx.close()
+
+
+def test_dslash_apply_is_asynchronous_on_its_stream(B):
+    """include/clover.h: dslash_apply is "Asynchronous on `stream`".  With the workspaces in place a call on one stream must
+    return while a long kernel queued on ANOTHER stream is still running (no device-wide synchronisation inside the call), and
+    two calls on two streams give the same result as on the default stream."""
+    c = wl.CONFIGS[1]
+    S = Setup(B, c["dims"], c["eps"], c["kappa"], c["csw"], c["gauge_seed"])
+    psi = B.noise_fill(c["dims"], 11, 4, scale=1.0)
+    want = S.ctx.dslash_apply(B.OP_D_FULL, psi)          # also allocates the workspaces
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    blocker_done = torch.cuda.Event()
+    with torch.cuda.stream(s1):
+        torch.cuda._sleep(int(3e9))                      # ~1.5 s of spinning on s1
+        blocker_done.record(s1)
+    with torch.cuda.stream(s2):
+        got = S.ctx.dslash_apply(B.OP_D_FULL, psi)
+        mine = torch.cuda.Event()
+        mine.record(s2)
+    returned_early = not blocker_done.query()
+    mine.synchronize()
+    finished_early = not blocker_done.query()            # the whole op ran to completion beside the blocker
+    torch.cuda.synchronize()
+    assert returned_early and finished_early
+    assert torch.equal(got, want)
+    S.ctx.close()
