@@ -48,6 +48,7 @@ struct clover_ctx {
     // scratch fields (internal layout) sized for max_rhs, allocated lazily by the solver / bench / dslash_apply
     clv::SolveWork *work;
     clover_solve_stats stats;
+    unsigned *sched;             // two device counters (zeroed) of the persistent Dslash kernels' tile scheduler; they leave them zeroed
     std::vector<void *> allocs;  // every device allocation of the operator data (freed by clover_destroy)
 };
 

@@ -84,23 +84,127 @@ __device__ __forceinline__ void hop_gather3(const Geom &g, const float4 *__restr
     d.neg = wrap && g.bc[MU] < 0;
 }
 
+// Own-site streams of the epilogue (x, w): no prefetch.  (The pair kernel prefetches them into L1 at kernel start; here the L1 is smaller
+// by the record buffers and the lines do not survive the hop: measured at 24^3x48, s epilogue 254 us with, 245 us without.)
+#ifndef CLV_R3_PF
+#define CLV_R3_PF 0   // 0 none, 1 prefetch.L1 at tile start, 2 prefetch.L2 at tile start, 3 prefetch.L1 after direction 3
+#endif
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+template <int XMODE, int DOT, int LEVEL> __device__ __forceinline__ void prefetch_own_site(const DslashArgs<float> &a, unsigned j)
+{
+    if (XMODE != XM_NONE) {
+        const float4 *q = a.xin + lb_index(j, 0, 6);
+#pragma unroll
+        for (int k = 0; k < 6; k++) { if (LEVEL == 1) prefetch_l1(q + 32 * k); else prefetch_l2(q + 32 * k); }
+    }
+    if (DOT == DOT_W || DOT == DOT_RES || DOT == DOT_S || DOT == DOT_XW) {
+        const float4 *q = a.w + lb_index(j, 0, 6);
+#pragma unroll
+        for (int k = 0; k < 6; k++) { if (LEVEL == 1) prefetch_l1(q + 32 * k); else prefetch_l2(q + 32 * k); }
+    }
+}
+
+// per-tile partial sums of one rhs in fp32 (the 12 terms of a site; same definitions as dots<> in dslash2_kernel.cuh)
+template <int DOT> __device__ __forceinline__ void dots_f(const cx<float> acc[12], const cx<float> x[12], const cx<float> w[12], float *f)
+{
+    if (DOT == DOT_W) {
+        float f0 = 0.f, f1 = 0.f;
+#pragma unroll
+        for (int i = 0; i < 12; i++) {  // <w, out>
+            f0 += w[i].re * acc[i].re + w[i].im * acc[i].im;
+            f1 += w[i].re * acc[i].im - w[i].im * acc[i].re;
+        }
+        f[0] = f0; f[1] = f1; f[2] = 0.f;
+    }
+    if (DOT == DOT_RES) {  // acc already holds w - (...)
+        float f0 = 0.f;
+#pragma unroll
+        for (int i = 0; i < 12; i++) f0 += acc[i].re * acc[i].re + acc[i].im * acc[i].im;
+        f[0] = f0; f[1] = 0.f; f[2] = 0.f;
+    }
+    if (DOT == DOT_X || DOT == DOT_XW) {
+        float f0 = 0.f, f1 = 0.f, f2 = 0.f;
+#pragma unroll
+        for (int i = 0; i < 12; i++) {  // <out, xin>, <out, out>
+            f0 += acc[i].re * x[i].re + acc[i].im * x[i].im;
+            f1 += acc[i].re * x[i].im - acc[i].im * x[i].re;
+            f2 += acc[i].re * acc[i].re + acc[i].im * acc[i].im;
+        }
+        f[0] = f0; f[1] = f1; f[2] = f2;
+    }
+    if (DOT == DOT_XW) {
+        float f3 = 0.f, f4 = 0.f, f5 = 0.f, f6 = 0.f;
+#pragma unroll
+        for (int i = 0; i < 12; i++) {  // <w, out>, <w, xin>
+            f3 += w[i].re * acc[i].re + w[i].im * acc[i].im;
+            f4 += w[i].re * acc[i].im - w[i].im * acc[i].re;
+            f5 += w[i].re * x[i].re + w[i].im * x[i].im;
+            f6 += w[i].re * x[i].im - w[i].im * x[i].re;
+        }
+        f[3] = f3; f[4] = f4; f[5] = f5; f[6] = f6;
+    }
+}
+
+// Reduce-scatter of a warp tile's partial sums (B = 8, one-warp CTAs: lane = 4 site + pair, 8 sites x 4 rhs pairs).  v holds the NV = 2 ND
+// sums of this thread's two rhs, padded to 8 K values (K = 1 | 2).  Three butterfly steps over the site bits of the lane, each sending one
+// half of the values and keeping the other, leave lane (site s, pair q) with the sums over the tile's 8 sites of values K s .. K s + K - 1 of
+// pair q: 7 or 14 shuffles instead of 3 NV, and K accumulators per thread instead of NV -- the hop has no registers for more.
+// (The 8 sites of a tile are summed in fp32, tiles in fp64; fixed order: deterministic.)
+template <int K> __device__ __forceinline__ void reduce_scatter_sites(float (&v)[8 * K], float (&out)[K])
+{
+    const unsigned lane = threadIdx.x & 31u;
+    float h4[4 * K], h2[2 * K];
+    {
+        const bool up = lane & 16u;
+#pragma unroll
+        for (int i = 0; i < 4 * K; i++) {
+            const float send = up ? v[i] : v[4 * K + i], keep = up ? v[4 * K + i] : v[i];
+            h4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+        }
+    }
+    {
+        const bool up = lane & 8u;
+#pragma unroll
+        for (int i = 0; i < 2 * K; i++) {
+            const float send = up ? h4[i] : h4[2 * K + i], keep = up ? h4[2 * K + i] : h4[i];
+            h2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+        }
+    }
+    {
+        const bool up = lane & 4u;
+#pragma unroll
+        for (int i = 0; i < K; i++) {
+            const float send = up ? h2[i] : h2[K + i], keep = up ? h2[K + i] : h2[i];
+            out[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+        }
+    }
+}
+
+// The CTA (one warp: 8 consecutive sites x 4 rhs pairs) loops over tiles with two record buffers, the records of the next tile posted when a
+// tile starts.  Tiles are handed out in order by an atomic counter (`sched[0]`; the first gridDim.x tiles statically), not round-robin: CTAs
+// that fall behind would otherwise spread the window of sites in flight over many timeslices and the neighbour gathers would stop hitting L2
+// (measured at 32^3x64: a round-robin assignment lost everything the records had gained).  The last CTA to leave re-arms the counters for
+// the next launch.  Dot-product variants leave ONE line of partial sums per CTA for the whole launch.
 template <int B, int RECON, int XMODE, int PINV, int DOT, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, CLV_R3_CTAS_PER_SM_WARPS * 32 / BLOCK)
-dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
+dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, unsigned *__restrict__ sched)
 {
-    static_assert(B >= 2 && B % 2 == 0, "pairs of right-hand sides");
+    static_assert(B == 8 && BLOCK == 32, "lane = 4 site + pair");
     constexpr int SITES = 2 * BLOCK / B;          // sites of a CTA tile: consecutive cb
     constexpr int LREC = 8 * RECON;               // floats of a site's link record
     constexpr bool CLOV = (XMODE == XM_CLOVER || PINV);
-    constexpr int ND = DOT == DOT_XW ? 7 : 3;
+    constexpr bool RED = (DOT != DOT_NONE && DOT != DOT_S);
+    constexpr int ND = DOT == DOT_XW ? 7 : 3;     // sums per rhs
+    constexpr int K = DOT == DOT_XW ? 2 : 1;      // accumulators per thread after the reduce-scatter: values K s .. K s + K - 1 of (2 ND padded to 8 K)
     __shared__ __align__(128) float lk_s[2][SITES * LREC];
     __shared__ __align__(128) float4 cl_s[2][CLOV ? SITES * 18 : 1];
     __shared__ __align__(8) unsigned long long bar[2];
+    __shared__ unsigned next_s[2];
     const int p = a.parity;
     const float *lk_g = p ? op.pk_link[1] : op.pk_link[0];
     const float *cl_g = PINV ? (p ? op.pk_clov_inv[1] : op.pk_clov_inv[0]) : (p ? op.pk_clov[1] : op.pk_clov[0]);
     const unsigned ntiles = ((unsigned)g.Vh + SITES - 1) / SITES;
-    // one thread posts the record of a tile: links and (if this variant applies A or A^-1) clover blocks, one bulk copy each
+    // one thread posts the records of a tile: its links and (if this variant applies A or A^-1) its clover blocks, one bulk copy each
     auto post = [&](unsigned tile, int buf) {
         const unsigned cb0 = tile * SITES, ns = min((unsigned)SITES, (unsigned)g.Vh - cb0);
         mbar_expect_tx(&bar[buf], ns * (LREC * 4u + (CLOV ? 288u : 0u)));
@@ -113,14 +217,20 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (threadIdx.x == 0 && blockIdx.x < ntiles) post(blockIdx.x, 0);
-    double dA[ND] = {}, dB[ND] = {};
-    unsigned it = 0;
-    for (unsigned tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+    unsigned it = 0, tile = blockIdx.x;   // (the grid never exceeds the tiles)
+    if (threadIdx.x == 0) post(tile, 0);
+    double sum[K] = {};
+    do {
         const int buf = it & 1;
-        if (threadIdx.x == 0 && tile + gridDim.x < ntiles) post(tile + gridDim.x, buf ^ 1);   // buf^1 was released by the barrier that ended iteration it-1
+        const unsigned par = (it >> 1) & 1;
+        if (threadIdx.x == 0) {   // fetch the next tile and post its records; buf^1 was released by the barrier that ended iteration it-1
+            const unsigned nt = gridDim.x + atomicAdd(&sched[0], 1u);
+            next_s[buf] = nt;
+            if (nt < ntiles) post(nt, buf ^ 1);
+        }
         const unsigned j = 2u * (tile * BLOCK + threadIdx.x);   // first rhs of this thread's pair
         const bool active = j < (unsigned)g.Vh * B;
+        float v[8 * K] = {};
         if (active) {
             const int cb = j / B, rhs = j % B;
             const int site = cb - tile * SITES;
@@ -128,15 +238,16 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
             HopAcc<float> hA, hB;
             hA.zero();
             hB.zero();
-            prefetch_epilogue<float, (XMODE == XM_CLOVER ? XM_PLAIN : XMODE), 0, DOT>(op, a, p, cb, j);   // x and w lines (the pair shares them)
+            if (CLV_R3_PF == 1 || CLV_R3_PF == 2) prefetch_own_site<XMODE, DOT, CLV_R3_PF>(a, j);   // x and w lines (the pair shares them)
             const float *rec = &lk_s[buf][site * LREC];
             {
                 HopIn2 d;
                 hop_gather3<B, 0, 1>(g, a.in, cb, rhs, c, d);
-                mbar_wait(&bar[buf], (it >> 1) & 1);   // this tile's record has landed (posted one tile ahead)
+                mbar_wait(&bar[buf], par);   // this tile's records have landed (posted one tile ahead)
 #define CLV_HOP3(MU, FW) lds_link<RECON, 2 * MU + 1 - FW>(rec, d.u); hop_compute2<RECON, MU, FW>(d, hA, hB);
 #define CLV_GAT3(MU, FW) hop_gather3<B, MU, FW>(g, a.in, cb, rhs, c, d);
                 CLV_HOP3(0, 1) CLV_GAT3(0, 0) CLV_HOP3(0, 0) CLV_GAT3(1, 1) CLV_HOP3(1, 1) CLV_GAT3(1, 0) CLV_HOP3(1, 0)
+                if (CLV_R3_PF == 3) prefetch_own_site<XMODE, DOT, 1>(a, j);
                 CLV_GAT3(2, 1) CLV_HOP3(2, 1) CLV_GAT3(2, 0) CLV_HOP3(2, 0) CLV_GAT3(3, 1) CLV_HOP3(3, 1) CLV_GAT3(3, 0) CLV_HOP3(3, 0)
 #undef CLV_HOP3
 #undef CLV_GAT3
@@ -171,13 +282,11 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
             }
             cx<float> wA[12], wB[12];
             if (DOT == DOT_W || DOT == DOT_RES || DOT == DOT_S || DOT == DOT_XW) load_spinor2(a.w, j, wA, wB);
-            if (DOT == DOT_RES) {  // result = w - acc, ||result||^2 (fp32 iteration precision: out32 and out are the same type here)
+            if (DOT == DOT_RES) {  // result = w - acc (fp32 iteration precision: out32 and out are the same type here)
 #pragma unroll
                 for (int i = 0; i < 12; i++) {
                     accA[i] = wA[i] - accA[i];
                     accB[i] = wB[i] - accB[i];
-                    dA[0] += (double)accA[i].re * (double)accA[i].re + (double)accA[i].im * (double)accA[i].im;
-                    dB[0] += (double)accB[i].re * (double)accB[i].re + (double)accB[i].im * (double)accB[i].im;
                 }
             }
             if (DOT != DOT_S) store_spinor2((DOT == DOT_RES && a.out32) ? a.out32 : a.out, j, accA, accB);
@@ -191,15 +300,39 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a)
                 }
                 store_spinor2(a.out2, j, wA, wB);
             }
-            dots<DOT>(accA, xA, wA, dA);
-            dots<DOT>(accB, xB, wB, dB);
+            if (RED) {
+                dots_f<DOT>(accA, xA, wA, v);
+                dots_f<DOT>(accB, xB, wB, v + ND);
+            }
         } else {
-            mbar_wait(&bar[buf], (it >> 1) & 1);
+            mbar_wait(&bar[buf], par);
         }
-        __syncthreads();   // every read of this tile's record is done before the buffer is posted again
+        if (RED) {
+            float t[K];
+            reduce_scatter_sites<K>(v, t);
+#pragma unroll
+            for (int k = 0; k < K; k++) sum[k] += (double)t[k];
+        }
+        __syncthreads();   // every read of this tile's records is done before the buffer is posted again
+        tile = next_s[buf];
+        it++;
+    } while (tile < ntiles);
+    if (threadIdx.x == 0) {   // the last CTA to finish re-arms the tile counter for the next launch on this context
+        __threadfence();
+        if (atomicInc(&sched[1], gridDim.x - 1) == gridDim.x - 1) sched[0] = 0;
     }
-    // one line of partial sums per CTA for the whole launch (fixed tile -> CTA assignment and summation order: deterministic)
-    if (DOT != DOT_NONE && DOT != DOT_S) block_reduce_pair<B, BLOCK, ND>(dA, dB, a.partial, a.partial2);
+    if (RED) {   // lane (site s, pair q) holds values K s .. K s + K - 1 of pair q: value c < ND belongs to rhs 2q, else c - ND to rhs 2q + 1
+        const int s = threadIdx.x >> 2, q = threadIdx.x & 3;
+#pragma unroll
+        for (int k = 0; k < K; k++) {
+            const int cidx = K * s + k;
+            if (cidx < 2 * ND) {
+                const int r = 2 * q + (cidx >= ND), cc = cidx % ND;
+                if (cc < 3) a.partial[((size_t)blockIdx.x * B + r) * 4 + cc] = sum[k];
+                else a.partial2[((size_t)blockIdx.x * B + r) * 4 + (cc - 3)] = sum[k];
+            }
+        }
+    }
 }
 
 }  // namespace clv

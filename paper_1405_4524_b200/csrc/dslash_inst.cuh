@@ -43,7 +43,9 @@ static int launch_dslash2_BR(const clover_ctx *ctx, const OpData<float> &op, con
     CLV_CUDA(cudaGetLastError());
     return 0;
 }
-// fp32, B = 8: the persistent kernel of dslash3_kernel.cuh (operator data by bulk async copy); grid = resident CTAs of the device
+// fp32, B = 8: the persistent kernel of dslash3_kernel.cuh (operator data by bulk async copy): grid = the one-warp CTAs resident on the
+// device.  The shared-memory carveout is set to what the resident CTAs need (+1 KB per CTA the system reserves) so that the rest of the
+// SM's 228 KB stays L1 for the gathers.
 template <int B, int RECON>
 static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
 {
@@ -52,14 +54,21 @@ static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, con
     const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
 #define CLV_LAUNCH3(XM, PI, DT)                                                                                          \
     case (XM) * 100 + (PI) * 10 + (DT): {                                                                                \
-        constexpr int BLK = CLV_HAS_RED(DT) ? CLV_R2_BLOCK_DOT : CLV_R2_BLOCK_NODOT;                                     \
+        constexpr int BLK = 32;                                                                                          \
+        constexpr int RESIDENT = CLV_R3_CTAS_PER_SM_WARPS * 32 / BLK;                                                    \
         auto kern = dslash3_kernel<B, RECON, XM, PI, DT, BLK>;                                                           \
-        static const cudaError_t attr = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
+        static const cudaError_t attr = [&] {                                                                            \
+            cudaFuncAttributes fa;                                                                                       \
+            cudaError_t e = cudaFuncGetAttributes(&fa, kern);                                                            \
+            if (e != cudaSuccess) return e;                                                                              \
+            const int pct = std::min<int>(100, (int)((fa.sharedSizeBytes + 1024) * RESIDENT * 100 / (228 * 1024)) + 3);  \
+            return cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct);                      \
+        }();                                                                                                             \
         CLV_CUDA(attr);                                                                                                  \
         const unsigned ntiles = ((unsigned)g.Vh + (2 * BLK / B) - 1) / (2 * BLK / B);                                    \
-        const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * (CLV_R3_CTAS_PER_SM_WARPS * 32 / BLK));        \
+        const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * RESIDENT);                                     \
         if (grid_out) *grid_out = (int)grid;                                                                             \
-        kern<<<grid, BLK, 0, st>>>(g, op, a);                                                                            \
+        kern<<<grid, BLK, 0, st>>>(g, op, a, ctx->sched);                                                                \
         break;                                                                                                           \
     }
     switch (key) {
@@ -102,7 +111,7 @@ template <int RECON> struct PairLaunch<float, 4, RECON> : PairLaunchF<4, RECON> 
 template <int RECON> struct PairLaunch<float, 8, RECON> : PairLaunchF<8, RECON> {
     static int go(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
     {
-        static const bool r3 = [] { const char *e = getenv("CLOVER_R3"); return e ? atoi(e) != 0 : false; }();  // tuning/debug knob only
+        static const bool r3 = [] { const char *e = getenv("CLOVER_R3"); return e ? atoi(e) != 0 : true; }();  // tuning/debug knob only
         return r3 ? launch_dslash3_BR<8, RECON>(ctx, op, a, st, grid_out) : launch_dslash2_BR<8, RECON>(ctx, op, a, st, grid_out);
     }
 };
@@ -112,7 +121,8 @@ template <typename R, int B, int RECON>
 static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const DslashArgs<R> &a, cudaStream_t st, int *grid_out)
 {
     // the pair kernel wins where link AND clover loads are shared (the fused solver kernels); the plain hop stays per-rhs
-    if (PairLaunch<R, B, RECON>::use() && (a.xmode != XM_NONE || a.pinv)) return PairLaunch<R, B, RECON>::go(ctx, op, a, st, grid_out);
+    static const bool hop3 = [] { const char *e = getenv("CLOVER_R3_HOP"); return e ? atoi(e) != 0 : false; }();  // tuning/debug knob only
+    if (PairLaunch<R, B, RECON>::use() && (a.xmode != XM_NONE || a.pinv || (hop3 && B == 8))) return PairLaunch<R, B, RECON>::go(ctx, op, a, st, grid_out);
     const Geom &g = ctx->geom;
     const unsigned n = (unsigned)g.Vh * B;
     const unsigned block = CLV_HAS_RED(a.dot) ? DSLASH_BLOCK : CLV_DSLASH_BLOCK_NODOT;

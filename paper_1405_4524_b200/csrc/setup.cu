@@ -384,6 +384,7 @@ int setup_operator(clover_ctx *ctx, const double *gauge_dev, cudaStream_t st)
         CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov[p], (size_t)g.Vh * 72, st));
         CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov_inv[p], (size_t)g.Vh * 72, st));
     }
+    CLV_CHECK(dev_alloc(ctx, &ctx->sched, 2, st));
     int *singular = nullptr;
     CLV_CHECK(dev_alloc(ctx, &singular, 1, st));
     dim3 gg((g.Vh + 127) / 128, 8);
