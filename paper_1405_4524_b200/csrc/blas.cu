@@ -263,6 +263,7 @@ __device__ __forceinline__ bool finite_z(zs z) { return isfinite(z.re) && isfini
 
 // one block per rhs: sum partial[(b*B + rhs)*4 + c] over b < nblocks in a fixed order, then thread 0 updates the scalars.
 constexpr int SC_SLICES = 32;
+constexpr int LEG_MAX = 48;   // sloppy iterations between two reliable updates at most (the benchmarked systems need 12-14 per leg)
 __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblocks, const double *__restrict__ partial, const double *__restrict__ partial2,
                                                      RhsScalars *sc, double tol2, double delta2, double *stage, unsigned *ticket, RhsScalars *publish)
 {
@@ -340,6 +341,8 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         q.claim = 0;
         q.restart = 0;
         q.nrestart = 0;
+        q.delta2 = delta2;
+        q.since = 0;
         if (!(q.eta2 > 0.) || d0 <= tol2 * q.eta2) q.done = 1;  // zero source or already converged
         if (!isfinite(d0)) { q.done = 1; q.status = 3; }
         if (step == SC_INIT_MERGED && !q.done) q.restart = 1;  // merged iteration: the start is a restart of every active rhs (SC_RESTART2)
@@ -381,7 +384,7 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             if (d2 > q.maxr2) q.maxr2 = d2;
             if (!isfinite(d2) || !finite_z(rho1)) { q.done = 1; q.status = 3; }
             else {
-                if (d2 < delta2 * q.maxr2) q.want_update = 1;
+                if (d2 < q.delta2 * q.maxr2 || ++q.since >= LEG_MAX) q.want_update = 1;
                 q.claim = (d2 <= tol2 * q.eta2) ? 1 : 0;
                 const double om2 = om.re * om.re + om.im * om.im, rh2 = rho.re * rho.re + rho.im * rho.im;
                 if (!(om2 > 0.) || !(rh2 > 0.)) q.want_update = 1;  // stagnation: let the fp64 residual decide, beta = 0 restarts p = r
@@ -397,6 +400,11 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         q.true_r2 = d0;
         q.claim = 0;
         if (!q.done) {
+            // The leg that just ended started at max||r||^2 = maxr2 and claims the iterated q.r2.  If the true residual is more than twice the
+            // claim, the sloppy precision gave out before the leg's target: ask the next legs for no more than four times (in ||r||) what
+            // this one really achieved, never for less than a factor 10, never for more than the solver's delta.
+            if (isfinite(d0) && d0 > 4. * q.r2 && q.maxr2 > 0.) q.delta2 = fmin(1e-2, fmax(q.delta2, 16. * d0 / q.maxr2));
+            q.since = 0;
             q.r2 = q.maxr2 = d0;
             q.want_update = 0;
             if (!isfinite(d0)) { q.done = 1; q.status = 3; }
@@ -442,7 +450,7 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             if (d2 > q.maxr2) q.maxr2 = d2;
             if (!isfinite(d2) || !isfinite(d0) || !isfinite(d1)) { q.done = 1; q.status = 3; }
             else {
-                if (d2 < delta2 * q.maxr2) q.want_update = 1;
+                if (d2 < q.delta2 * q.maxr2 || ++q.since >= LEG_MAX) q.want_update = 1;
                 q.claim = (d2 <= tol2 * q.eta2) ? 1 : 0;
                 if (q.restart != 1) {  // (a restart recomputes alpha itself)
                     if (d0 * d0 + d1 * d1 > 0.) al = zdiv(ld_z(q.rho), zs{d0, d1});

@@ -33,6 +33,13 @@ struct RhsScalars {
     int claim;        // 1 if the iterated residual of this rhs meets the tolerance (to be confirmed in fp64)
     int restart;      // 1 if <r0, v> vanished this iteration: r0 := r, rho := ||r||^2 before the next one (R11)
     int nrestart;     // restarts so far (a rhs that keeps breaking down ends with status 2)
+    // reliable-update control of this rhs (R11): a leg of sloppy iterations ends when ||r||^2 < delta2 * max||r||^2, or after LEG_MAX
+    // iterations.  delta2 starts at the solver's delta^2 and is RAISED when a reliable update finds the true residual well above the
+    // iterated one (the leg asked the sloppy precision for more than it can deliver: ill-conditioned systems), so that the next legs
+    // stop where the sloppy residual is still true.
+    double delta2;
+    int since;        // sloppy iterations since the last reliable update
+    int pad_;
 };
 
 struct SolveWork;  // solver.cu

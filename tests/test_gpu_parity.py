@@ -277,3 +277,34 @@ def test_dslash_apply_is_asynchronous_on_its_stream(B):
     assert returned_early and finished_early
     assert torch.equal(got, want)
     S.ctx.close()
+
+
+@pytest.mark.parametrize("dims,eps", [((4, 4, 4, 8), 0.4), ((8, 8, 8, 16), 0.4), ((8, 8, 8, 16), 0.5)])
+def test_solve_at_the_papers_parameter_point(B, dims, eps):
+    """The paper's own point: kappa = 0.13514 (m0 a = -0.300), c_sw = 1.0, periodic in all four directions, on rough
+    synthetic links, 8 sources, mixed precision.  These systems are far worse conditioned than BASELINE.json's (hundreds of
+    iterations instead of 25): the fp32 legs cannot deliver the solver's default delta, so this is the test that the reliable
+    updates (adaptive per-rhs delta, R11) still converge to 1e-10 and that the result is the oracle's.  With
+    cond(D) ~ 1e3 a residual of 1e-10 bounds the solution error only by ~1e-7, so the 1e-8 solution bar is checked on a solve to
+    1e-12 (both sides), and the 1e-10 solve is held to cond(D) * residual with the oracle-solved solution as the reference."""
+    kappa, csw, bc = 0.13514, 1.0, (1, 1, 1, 1)
+    S = Setup(B, dims, eps, kappa, csw, seed=77, bc=bc)
+    eta = B.noise_fill(dims, 5, 8, scale=wl.INV_SQRT2)
+    e = eta.cpu().numpy()
+    want, oi = oracle.bicgstab(S.U, S.A, bc, kappa, e[0], tol=1e-13, max_iter=20000)
+    assert oi["status"] == 0
+    for tol, bar in ((1e-10, 1e-6), (1e-12, 1e-8)):
+        psi, infos, bad = S.ctx.solve(eta, tol=tol, batch=8, mixed=True, max_iter=5000)
+        assert bad == 0, infos
+        p = psi.cpu().numpy()
+        for r in range(8):
+            res = np.linalg.norm(e[r] - oracle.apply_D(S.U, S.A, bc, kappa, p[r])) / np.linalg.norm(e[r])
+            assert infos[r]["status"] == 0 and res <= tol and abs(infos[r]["true_resid"] - res) <= 1e-3 * res + 1e-14, (r, res, infos[r])
+        err = np.linalg.norm(p[0] - want) / np.linalg.norm(want)
+        assert err < bar and nerr(p[0], want) < bar, (tol, err)
+        # fp32 rounding perturbs the Krylov recurrence of so badly conditioned a system, so the mixed solve needs more iterations than
+        # the all-fp64 one (measured: 336 against 180 on 4^3x8, 351 against 281 on 8^3x16 at eps 0.4; equal counts at eps 0.5; with
+        # the constant delta of round 1: 425 and 437): the adaptive delta must keep it within 2.5 x
+        _, infos64, bad64 = S.ctx.solve(eta, tol=tol, batch=8, mixed=False, max_iter=5000)
+        assert bad64 == 0 and infos[0]["iters"] <= 2.5 * infos64[0]["iters"] + 20, (infos[0], infos64[0])
+    S.ctx.close()
