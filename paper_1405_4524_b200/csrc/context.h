@@ -14,10 +14,18 @@ template <typename R> struct OpData {
     C *clov_inv[2];   // A^-1, same packing
     int recon;        // 18 | 12
     // Site-major ("packed") copies for the B = 8 kernels, fetched per CTA tile with one bulk async copy each (dslash3_kernel.cuh):
+    // Records are padded (pk_link_stride / PK_CLOV_STRIDE reals per site) so that in shared memory the 8 sites of a warp tile fall into
+    // disjoint 4-bank groups: a warp-wide 16-byte load of "the same element of 8 sites" is then one conflict-free wavefront.
     R *pk_link[2];     // [parity p of the OUTPUT site][cb][d = 2 mu + (fwd ? 0 : 1)][recon reals]: fwd = U_mu(x), bwd = U_mu(x - mu) as stored
     R *pk_clov[2];     // [parity][cb][72 reals]: the 18 16-byte rows (fp32) of the packed blocks of A
     R *pk_clov_inv[2]; // A^-1
 };
+// reals per site record: 8 links of `recon` reals + 4 of padding (592 or 400 bytes in fp32: 20 s or 4 s words mod 32 for site s), 72 + 4 for the clover blocks
+#ifndef CLV_PK_PAD
+#define CLV_PK_PAD 4
+#endif
+__host__ __device__ constexpr int pk_link_stride(int recon) { return 8 * recon + CLV_PK_PAD; }
+constexpr int PK_CLOV_STRIDE = 72 + CLV_PK_PAD;
 
 // Per-rhs solver scalars, device resident (one entry per rhs of the batch).
 struct RhsScalars {

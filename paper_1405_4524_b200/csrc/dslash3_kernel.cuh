@@ -15,6 +15,9 @@
 
 namespace clv {
 
+#ifndef CLV_R3_PFT
+#define CLV_R3_PFT 1   // L2 prefetch of the tile's forward-t neighbour lines when the tile starts
+#endif
 #ifndef CLV_R3_CTAS_PER_SM_WARPS
 #define CLV_R3_CTAS_PER_SM_WARPS 12   // resident warps per SM (168 registers per thread)
 #endif
@@ -180,70 +183,103 @@ template <int K> __device__ __forceinline__ void reduce_scatter_sites(float (&v)
     }
 }
 
-// The CTA (one warp: 8 consecutive sites x 4 rhs pairs) loops over tiles with two record buffers, the records of the next tile posted when a
-// tile starts.  Tiles are handed out in order by an atomic counter (`sched[0]`; the first gridDim.x tiles statically), not round-robin: CTAs
+// The CTA (one warp: 8 consecutive sites x 4 rhs pairs) loops over tiles.  The link records are double-buffered (the next tile's are posted when
+// a tile starts); the clover records have ONE buffer, re-posted for the next tile as soon as this tile's A / A^-1 product has read it -- the
+// copy then has the whole hop of the next tile to land.  Shared memory is kept small on purpose: what the records do not take stays L1, and
+// L1 capacity bounds the bytes the gathers can have in flight (measured at 24^3x48: the same kernel with 32 instead of 64 KB of L1 is 25 %
+// slower).  Tiles are handed out in order by an atomic counter (`sched[0]`; the first gridDim.x tiles statically), not round-robin: CTAs
 // that fall behind would otherwise spread the window of sites in flight over many timeslices and the neighbour gathers would stop hitting L2
 // (measured at 32^3x64: a round-robin assignment lost everything the records had gained).  The last CTA to leave re-arms the counters for
 // the next launch.  Dot-product variants leave ONE line of partial sums per CTA for the whole launch.
+#ifndef CLV_R3_CBUF
+#define CLV_R3_CBUF 1
+#endif
 template <int B, int RECON, int XMODE, int PINV, int DOT, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, CLV_R3_CTAS_PER_SM_WARPS * 32 / BLOCK)
 dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, unsigned *__restrict__ sched)
 {
     static_assert(B == 8 && BLOCK == 32, "lane = 4 site + pair");
     constexpr int SITES = 2 * BLOCK / B;          // sites of a CTA tile: consecutive cb
-    constexpr int LREC = 8 * RECON;               // floats of a site's link record
+    constexpr int LREC = pk_link_stride(RECON);   // floats of a site's (padded) link record
+    constexpr int CREC = PK_CLOV_STRIDE;          // floats of a site's (padded) clover record
     constexpr bool CLOV = (XMODE == XM_CLOVER || PINV);
     constexpr bool RED = (DOT != DOT_NONE && DOT != DOT_S);
     constexpr int ND = DOT == DOT_XW ? 7 : 3;     // sums per rhs
     constexpr int K = DOT == DOT_XW ? 2 : 1;      // accumulators per thread after the reduce-scatter: values K s .. K s + K - 1 of (2 ND padded to 8 K)
+    constexpr int NCB = CLV_R3_CBUF;              // clover buffers
     __shared__ __align__(128) float lk_s[2][SITES * LREC];
-    __shared__ __align__(128) float4 cl_s[2][CLOV ? SITES * 18 : 1];
-    __shared__ __align__(8) unsigned long long bar[2];
+    __shared__ __align__(128) float cl_s[NCB][CLOV ? SITES * CREC : 4];
+    __shared__ __align__(8) unsigned long long bar[2], bar_c[NCB];
     __shared__ unsigned next_s[2];
     const int p = a.parity;
     const float *lk_g = p ? op.pk_link[1] : op.pk_link[0];
     const float *cl_g = PINV ? (p ? op.pk_clov_inv[1] : op.pk_clov_inv[0]) : (p ? op.pk_clov[1] : op.pk_clov[0]);
     const unsigned ntiles = ((unsigned)g.Vh + SITES - 1) / SITES;
-    // one thread posts the records of a tile: its links and (if this variant applies A or A^-1) its clover blocks, one bulk copy each
-    auto post = [&](unsigned tile, int buf) {
+    // one thread posts the records of a tile with one bulk copy each
+    auto post_links = [&](unsigned tile, int buf) {
         const unsigned cb0 = tile * SITES, ns = min((unsigned)SITES, (unsigned)g.Vh - cb0);
-        mbar_expect_tx(&bar[buf], ns * (LREC * 4u + (CLOV ? 288u : 0u)));
+        mbar_expect_tx(&bar[buf], ns * LREC * 4u);
         bulk_g2s(&lk_s[buf][0], lk_g + (size_t)cb0 * LREC, ns * LREC * 4u, &bar[buf]);
-        if (CLOV) bulk_g2s(&cl_s[buf][0], cl_g + (size_t)cb0 * 72, ns * 288u, &bar[buf]);
+    };
+    auto post_clover = [&](unsigned tile, int buf) {
+        const unsigned cb0 = tile * SITES, ns = min((unsigned)SITES, (unsigned)g.Vh - cb0);
+        mbar_expect_tx(&bar_c[buf], ns * CREC * 4u);
+        bulk_g2s(&cl_s[buf][0], cl_g + (size_t)cb0 * CREC, ns * CREC * 4u, &bar_c[buf]);
     };
     if (threadIdx.x == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
+#pragma unroll
+        for (int k = 0; k < NCB; k++) mbar_init(&bar_c[k], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     unsigned it = 0, tile = blockIdx.x;   // (the grid never exceeds the tiles)
-    if (threadIdx.x == 0) post(tile, 0);
+    if (threadIdx.x == 0) {
+        post_links(tile, 0);
+        if (CLOV) post_clover(tile, 0);
+    }
     double sum[K] = {};
     do {
-        const int buf = it & 1;
-        const unsigned par = (it >> 1) & 1;
-        if (threadIdx.x == 0) {   // fetch the next tile and post its records; buf^1 was released by the barrier that ended iteration it-1
+        const int buf = it & 1, cbuf = NCB == 2 ? buf : 0;
+        const unsigned par = (it >> 1) & 1, cpar = NCB == 2 ? par : (it & 1);
+        if (threadIdx.x == 0) {   // draw the next tile and post its links; buf^1 was released by the barrier that ended iteration it-1
+            // (drawing the ticket one tile earlier, so that nobody waits for the atomic, measured 2 % slower)
             const unsigned nt = gridDim.x + atomicAdd(&sched[0], 1u);
             next_s[buf] = nt;
-            if (nt < ntiles) post(nt, buf ^ 1);
+            if (nt < ntiles) {
+                post_links(nt, buf ^ 1);
+                if (CLOV && NCB == 2) post_clover(nt, buf ^ 1);
+            }
         }
         const unsigned j = 2u * (tile * BLOCK + threadIdx.x);   // first rhs of this thread's pair
         const bool active = j < (unsigned)g.Vh * B;
+        const int cb = j / B, rhs = j % B;
+        const int site = cb - tile * SITES;
         float v[8 * K] = {};
+        cx<float> accA[12], accB[12], xA[12], xB[12];
         if (active) {
-            const int cb = j / B, rhs = j % B;
-            const int site = cb - tile * SITES;
             const Coord c = decode(g, cb, p);
             HopAcc<float> hA, hB;
             hA.zero();
             hB.zero();
             if (CLV_R3_PF == 1 || CLV_R3_PF == 2) prefetch_own_site<XMODE, DOT, CLV_R3_PF>(a, j);   // x and w lines (the pair shares them)
+            if (CLV_R3_PFT) {
+                // Tiles are processed in order of cb (t slowest), so the forward-t neighbours are the frontier: nobody has read them yet
+                // and their gather, the seventh direction, is a DRAM miss.  Ask L2 for their lines now: lane (site, pair q) takes rows
+                // q, q + 4 of its site's neighbour.  (Measured: -4 %; the same for the next tile, or for the own-site streams: slower.)
+                bool wrap;
+                const int nbt = neighbour<3, 1>(g, cb, c, wrap);
+                const float4 *q4 = a.in + lb_index((unsigned)nbt * B, 0, 6);
+                const int q = rhs >> 1;
+                prefetch_l2(q4 + 32 * q);
+                if (q < 2) prefetch_l2(q4 + 32 * (q + 4));
+            }
             const float *rec = &lk_s[buf][site * LREC];
             {
                 HopIn2 d;
                 hop_gather3<B, 0, 1>(g, a.in, cb, rhs, c, d);
-                mbar_wait(&bar[buf], par);   // this tile's records have landed (posted one tile ahead)
+                mbar_wait(&bar[buf], par);   // this tile's links have landed (posted one tile ahead)
 #define CLV_HOP3(MU, FW) lds_link<RECON, 2 * MU + 1 - FW>(rec, d.u); hop_compute2<RECON, MU, FW>(d, hA, hB);
 #define CLV_GAT3(MU, FW) hop_gather3<B, MU, FW>(g, a.in, cb, rhs, c, d);
                 CLV_HOP3(0, 1) CLV_GAT3(0, 0) CLV_HOP3(0, 0) CLV_GAT3(1, 1) CLV_HOP3(1, 1) CLV_GAT3(1, 0) CLV_HOP3(1, 0)
@@ -252,8 +288,6 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
 #undef CLV_HOP3
 #undef CLV_GAT3
             }
-            const float4 *srow = &cl_s[buf][CLOV ? site * 18 : 0];
-            cx<float> accA[12], accB[12];
             hA.finish(accA);
             hB.finish(accB);
 #pragma unroll
@@ -261,7 +295,6 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
                 accA[i] = a.coef * accA[i];
                 accB[i] = a.coef * accB[i];
             }
-            cx<float> xA[12], xB[12];
             if (XMODE != XM_NONE) load_spinor2(a.xin, j, xA, xB);
             if (XMODE == XM_PLAIN) {
 #pragma unroll
@@ -270,16 +303,29 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
                     accB[i] = accB[i] + xB[i];
                 }
             }
-            if (XMODE == XM_CLOVER) clover_mul2<true>(nullptr, cb, srow, xA, accA, xB, accB);
-            if (PINV) {
-                cx<float> tA[12], tB[12];
-                clover_mul2<false>(nullptr, cb, srow, accA, tA, accB, tB);
+            if (CLOV) {
+                mbar_wait(&bar_c[cbuf], cpar);
+                const float4 *srow = reinterpret_cast<const float4 *>(&cl_s[cbuf][site * CREC]);
+                if (XMODE == XM_CLOVER) clover_mul2<true>(nullptr, cb, srow, xA, accA, xB, accB);
+                if (PINV) {
+                    cx<float> tA[12], tB[12];
+                    clover_mul2<false>(nullptr, cb, srow, accA, tA, accB, tB);
 #pragma unroll
-                for (int i = 0; i < 12; i++) {
-                    accA[i] = tA[i];
-                    accB[i] = tB[i];
+                    for (int i = 0; i < 12; i++) {
+                        accA[i] = tA[i];
+                        accB[i] = tB[i];
+                    }
                 }
             }
+        } else {
+            mbar_wait(&bar[buf], par);
+            if (CLOV) mbar_wait(&bar_c[cbuf], cpar);
+        }
+        if (CLOV && NCB == 1) {   // the clover buffer has been read: it takes the next tile's blocks while this tile is finished and the next one hops
+            __syncthreads();
+            if (threadIdx.x == 0 && next_s[buf] < ntiles) post_clover(next_s[buf], 0);
+        }
+        if (active) {
             cx<float> wA[12], wB[12];
             if (DOT == DOT_W || DOT == DOT_RES || DOT == DOT_S || DOT == DOT_XW) load_spinor2(a.w, j, wA, wB);
             if (DOT == DOT_RES) {  // result = w - acc (fp32 iteration precision: out32 and out are the same type here)
@@ -304,8 +350,6 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
                 dots_f<DOT>(accA, xA, wA, v);
                 dots_f<DOT>(accB, xB, wB, v + ND);
             }
-        } else {
-            mbar_wait(&bar[buf], par);
         }
         if (RED) {
             float t[K];
@@ -313,7 +357,7 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
 #pragma unroll
             for (int k = 0; k < K; k++) sum[k] += (double)t[k];
         }
-        __syncthreads();   // every read of this tile's records is done before the buffer is posted again
+        __syncthreads();   // every read of this tile's link records is done before the buffer is posted again
         tile = next_s[buf];
         it++;
     } while (tile < ntiles);

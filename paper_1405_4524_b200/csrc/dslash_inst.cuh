@@ -3,6 +3,7 @@
 #pragma once
 #include "dslash3_kernel.cuh"
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 
 namespace clv {
@@ -46,6 +47,18 @@ static int launch_dslash2_BR(const clover_ctx *ctx, const OpData<float> &op, con
 // fp32, B = 8: the persistent kernel of dslash3_kernel.cuh (operator data by bulk async copy): grid = the one-warp CTAs resident on the
 // device.  The shared-memory carveout is set to what the resident CTAs need (+1 KB per CTA the system reserves) so that the rest of the
 // SM's 228 KB stays L1 for the gathers.
+#ifndef CLV_R3_GRID_PER_SM
+#define CLV_R3_GRID_PER_SM 12   // persistent one-warp CTAs launched per SM (<= the resident limit of the launch bounds)
+#endif
+// smallest shared-memory carveout of sm_100 (KB) that holds `ctas` CTAs of `bytes` static shared memory + 1 KB each, as a percentage of 228 KB
+static int r3_carveout_pct(size_t bytes, int ctas)
+{
+    static const int kb[] = {8, 16, 32, 64, 100, 132, 164, 196, 228};
+    const size_t need = (bytes + 1024) * ctas;
+    for (int k : kb)
+        if ((size_t)k * 1024 >= need) return (k * 100 + 227) / 228;
+    return 100;
+}
 template <int B, int RECON>
 static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, const DslashArgs<float> &a, cudaStream_t st, int *grid_out)
 {
@@ -55,18 +68,23 @@ static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, con
 #define CLV_LAUNCH3(XM, PI, DT)                                                                                          \
     case (XM) * 100 + (PI) * 10 + (DT): {                                                                                \
         constexpr int BLK = 32;                                                                                          \
-        constexpr int RESIDENT = CLV_R3_CTAS_PER_SM_WARPS * 32 / BLK;                                                    \
         auto kern = dslash3_kernel<B, RECON, XM, PI, DT, BLK>;                                                           \
         static const cudaError_t attr = [&] {                                                                            \
             cudaFuncAttributes fa;                                                                                       \
             cudaError_t e = cudaFuncGetAttributes(&fa, kern);                                                            \
             if (e != cudaSuccess) return e;                                                                              \
-            const int pct = std::min<int>(100, (int)((fa.sharedSizeBytes + 1024) * RESIDENT * 100 / (228 * 1024)) + 3);  \
-            return cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, pct);                      \
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, r3_carveout_pct(fa.sharedSizeBytes, CLV_R3_GRID_PER_SM)); \
+            if (getenv("CLOVER_DEBUG_OCC")) {                                                                            \
+                int occ = -1;                                                                                            \
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLK, 0);                                       \
+                fprintf(stderr, "dslash3<%d,%d,%d> smem %zu regs %d carveout %d%% occupancy %d CTAs/SM\n", XM, PI, DT, fa.sharedSizeBytes, fa.numRegs, \
+                        r3_carveout_pct(fa.sharedSizeBytes, CLV_R3_GRID_PER_SM), occ);                                   \
+            }                                                                                                            \
+            return e;                                                                                                    \
         }();                                                                                                             \
         CLV_CUDA(attr);                                                                                                  \
         const unsigned ntiles = ((unsigned)g.Vh + (2 * BLK / B) - 1) / (2 * BLK / B);                                    \
-        const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * RESIDENT);                                     \
+        const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * CLV_R3_GRID_PER_SM);                           \
         if (grid_out) *grid_out = (int)grid;                                                                             \
         kern<<<grid, BLK, 0, st>>>(g, op, a, ctx->sched);                                                                \
         break;                                                                                                           \

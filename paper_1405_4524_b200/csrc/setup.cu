@@ -65,7 +65,7 @@ template <int RECON32> __global__ void pack_links_kernel(Geom g, const double *_
     const Lex x = lex_of(g, cb, p);
     zc u[9];
     ld_link(gauge, V, mu, lex_index(g, (d & 1) ? shifted(g, x, mu, -1) : x), u);
-    float2 *o = reinterpret_cast<float2 *>(o32.pk_link[p] + ((size_t)cb * 8 + d) * RECON32);
+    float2 *o = reinterpret_cast<float2 *>(o32.pk_link[p] + (size_t)cb * pk_link_stride(RECON32) + d * RECON32);
 #pragma unroll
     for (int k = 0; k < RECON32 / 2; k++) o[k] = make_float2((float)u[k].re, (float)u[k].im);
 }
@@ -78,7 +78,7 @@ __global__ void pack_clover_kernel(Geom g, OpData<float> o32)
     const int p = blockIdx.y >> 1;
     const float2 *src = (blockIdx.y & 1) ? o32.clov_inv[p] : o32.clov[p];
     float *dst = (blockIdx.y & 1) ? o32.pk_clov_inv[p] : o32.pk_clov[p];
-    reinterpret_cast<float4 *>(dst)[i] = __ldg(reinterpret_cast<const float4 *>(src) + ((size_t)(cb >> 5) * 18 + row) * 32 + (cb & 31u));
+    reinterpret_cast<float4 *>(dst + (size_t)cb * PK_CLOV_STRIDE)[row] = __ldg(reinterpret_cast<const float4 *>(src) + ((size_t)(cb >> 5) * 18 + row) * 32 + (cb & 31u));
 }
 
 // ---- S1: clover term ------------------------------------------------------------------------------
@@ -380,9 +380,9 @@ int setup_operator(clover_ctx *ctx, const double *gauge_dev, cudaStream_t st)
     }
     for (int p = 0; p < 2; p++) {
         ctx->op64.pk_link[p] = ctx->op64.pk_clov[p] = ctx->op64.pk_clov_inv[p] = nullptr;   // fp32 only
-        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_link[p], (size_t)g.Vh * 8 * ctx->op32.recon, st));
-        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov[p], (size_t)g.Vh * 72, st));
-        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov_inv[p], (size_t)g.Vh * 72, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_link[p], (size_t)g.Vh * pk_link_stride(ctx->op32.recon), st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov[p], (size_t)g.Vh * PK_CLOV_STRIDE, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov_inv[p], (size_t)g.Vh * PK_CLOV_STRIDE, st));
     }
     CLV_CHECK(dev_alloc(ctx, &ctx->sched, 2, st));
     int *singular = nullptr;
