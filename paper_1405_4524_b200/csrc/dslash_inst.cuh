@@ -2,6 +2,9 @@
 // dslash_<prec>_b<B>.cu instantiation units so the variants compile in parallel.
 #pragma once
 #include "dslash3_kernel.cuh"
+#ifdef CLV_BUILD_DSLASH3D   // defined by dslash_f64_b8.cu only: the fp64 B = 8 kernels are built once
+#include "dslash3d_kernel.cuh"
+#endif
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -109,6 +112,55 @@ static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, con
     return 0;
 }
 
+#ifdef CLV_BUILD_DSLASH3D
+// fp64, B = 8, the variants of the mixed-precision solve: dslash3d_kernel.cuh (persistent, one thread per site and rhs); false if not built
+static bool launch_dslash3d(const clover_ctx *ctx, const OpData<double> &op, const DslashArgs<double> &a, cudaStream_t st, int *grid_out, int *rc)
+{
+    const Geom &g = ctx->geom;
+    static const int n_sm = [] { int dev = 0, n = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); return n; }();
+    const int key = a.xmode * 100 + a.pinv * 10 + a.dot;
+    *rc = 0;
+#define CLV_LAUNCH3D(XM, PI, DT)                                                                                         \
+    case (XM) * 100 + (PI) * 10 + (DT): {                                                                                \
+        auto kern = dslash3d_kernel<XM, PI, DT>;                                                                         \
+        static const cudaError_t attr = [&] {                                                                            \
+            cudaFuncAttributes fa;                                                                                       \
+            cudaError_t e = cudaFuncGetAttributes(&fa, kern);                                                            \
+            if (e != cudaSuccess) return e;                                                                              \
+            return cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, r3_carveout_pct(fa.sharedSizeBytes, CLV_R3D_WARPS_PER_SM)); \
+        }();                                                                                                             \
+        if (attr != cudaSuccess) { set_error("cudaFuncSetAttribute failed: %s", cudaGetErrorString(attr)); *rc = CLOVER_ECUDA; return true; } \
+        const unsigned ntiles = ((unsigned)g.Vh + 3) / 4;                                                                \
+        const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * CLV_R3D_WARPS_PER_SM);                         \
+        if (grid_out) *grid_out = (int)grid;                                                                             \
+        kern<<<grid, 32, 0, st>>>(g, op, a, ctx->sched);                                                                 \
+        break;                                                                                                           \
+    }
+    switch (key) {
+        CLV_LAUNCH3D(XM_NONE, 1, DOT_NONE)
+        CLV_LAUNCH3D(XM_PLAIN, 0, DOT_NONE)
+        CLV_LAUNCH3D(XM_PLAIN, 1, DOT_NONE)
+        CLV_LAUNCH3D(XM_CLOVER, 0, DOT_RES)
+    default: return false;
+    }
+#undef CLV_LAUNCH3D
+    if (cudaGetLastError() != cudaSuccess) { set_error("dslash3d launch failed"); *rc = CLOVER_ECUDA; }
+    return true;
+}
+#endif
+template <typename R, int B> struct Launch3D {
+    static bool go(const clover_ctx *, const OpData<R> &, const DslashArgs<R> &, cudaStream_t, int *, int *) { return false; }
+};
+#ifdef CLV_BUILD_DSLASH3D
+template <> struct Launch3D<double, 8> {
+    static bool go(const clover_ctx *ctx, const OpData<double> &op, const DslashArgs<double> &a, cudaStream_t st, int *grid_out, int *rc)
+    {
+        static const bool on = [] { const char *e = getenv("CLOVER_R3D"); return e ? atoi(e) != 0 : true; }();  // tuning/debug knob only
+        return on && launch_dslash3d(ctx, op, a, st, grid_out, rc);
+    }
+};
+#endif
+
 template <typename R, int B, int RECON> struct PairLaunch {   // double, or B = 1: no pair kernel
     static bool use() { return false; }
     static int go(const clover_ctx *, const OpData<R> &, const DslashArgs<R> &, cudaStream_t, int *) { return CLOVER_EINVAL; }
@@ -141,6 +193,10 @@ static int launch_dslash_BR(const clover_ctx *ctx, const OpData<R> &op, const Ds
     // the pair kernel wins where link AND clover loads are shared (the fused solver kernels); the plain hop stays per-rhs
     static const bool hop3 = [] { const char *e = getenv("CLOVER_R3_HOP"); return e ? atoi(e) != 0 : false; }();  // tuning/debug knob only
     if (PairLaunch<R, B, RECON>::use() && (a.xmode != XM_NONE || a.pinv || (hop3 && B == 8))) return PairLaunch<R, B, RECON>::go(ctx, op, a, st, grid_out);
+    {
+        int rc3 = 0;
+        if (Launch3D<R, B>::go(ctx, op, a, st, grid_out, &rc3)) return rc3;
+    }
     const Geom &g = ctx->geom;
     const unsigned n = (unsigned)g.Vh * B;
     const unsigned block = CLV_HAS_RED(a.dot) ? DSLASH_BLOCK : CLV_DSLASH_BLOCK_NODOT;

@@ -54,9 +54,9 @@ __global__ void reorder_gauge_kernel(Geom g, const double *__restrict__ gauge, O
     for (int k = 0; k < RECON32 / 2; k++) o32.gauge[p][mu][cplx_index<float>(cb, k, RECON32 / 2)] = make_float2((float)u[k].re, (float)u[k].im);
 }
 
-// Site-major fp32 copies for the B = 8 kernels: per output site of parity p the 8 links of its hop, in the order d = 2 mu + (fwd ? 0 : 1)
-// (fwd: U_mu(x); bwd: U_mu(x - mu), stored as it is and daggered in-kernel), rounded to fp32 exactly as the lane-blocked copy is.
-template <int RECON32> __global__ void pack_links_kernel(Geom g, const double *__restrict__ gauge, OpData<float> o32)
+// Site-major copies for the B = 8 kernels: per output site of parity p the 8 links of its hop, in the order d = 2 mu + (fwd ? 0 : 1)
+// (fwd: U_mu(x); bwd: U_mu(x - mu), stored as it is and daggered in-kernel); fp32 rounded exactly as the lane-blocked copy is.
+template <typename R, int RECON> __global__ void pack_links_kernel(Geom g, const double *__restrict__ gauge, OpData<R> o)
 {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
@@ -65,20 +65,25 @@ template <int RECON32> __global__ void pack_links_kernel(Geom g, const double *_
     const Lex x = lex_of(g, cb, p);
     zc u[9];
     ld_link(gauge, V, mu, lex_index(g, (d & 1) ? shifted(g, x, mu, -1) : x), u);
-    float2 *o = reinterpret_cast<float2 *>(o32.pk_link[p] + (size_t)cb * pk_link_stride(RECON32) + d * RECON32);
+    R *dst = o.pk_link[p] + (size_t)cb * pk_link_stride(RECON) + d * RECON;
 #pragma unroll
-    for (int k = 0; k < RECON32 / 2; k++) o[k] = make_float2((float)u[k].re, (float)u[k].im);
+    for (int k = 0; k < RECON / 2; k++) {
+        dst[2 * k] = (R)u[k].re;
+        dst[2 * k + 1] = (R)u[k].im;
+    }
 }
-// lane-blocked rows of the packed clover blocks -> 18 consecutive 16-byte rows per site
-__global__ void pack_clover_kernel(Geom g, OpData<float> o32)
+// lane-blocked packed clover blocks (36 complex per site) -> 72 consecutive reals per site
+template <typename R> __global__ void pack_clover_kernel(Geom g, OpData<R> o)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= (unsigned)g.Vh * 18u) return;
-    const unsigned cb = i / 18u, row = i % 18u;
+    if (i >= (unsigned)g.Vh * 36u) return;
+    const unsigned cb = i / 36u, k = i % 36u;
     const int p = blockIdx.y >> 1;
-    const float2 *src = (blockIdx.y & 1) ? o32.clov_inv[p] : o32.clov[p];
-    float *dst = (blockIdx.y & 1) ? o32.pk_clov_inv[p] : o32.pk_clov[p];
-    reinterpret_cast<float4 *>(dst + (size_t)cb * PK_CLOV_STRIDE)[row] = __ldg(reinterpret_cast<const float4 *>(src) + ((size_t)(cb >> 5) * 18 + row) * 32 + (cb & 31u));
+    const typename Vec<R>::C *src = (blockIdx.y & 1) ? o.clov_inv[p] : o.clov[p];
+    R *dst = ((blockIdx.y & 1) ? o.pk_clov_inv[p] : o.pk_clov[p]) + (size_t)cb * PK_CLOV_STRIDE + 2 * k;
+    const typename Vec<R>::C v = src[cplx_index<R>(cb, k, 36)];
+    dst[0] = v.x;
+    dst[1] = v.y;
 }
 
 // ---- S1: clover term ------------------------------------------------------------------------------
@@ -379,7 +384,9 @@ int setup_operator(clover_ctx *ctx, const double *gauge_dev, cudaStream_t st)
         CLV_CHECK(dev_alloc(ctx, &ctx->op32.clov_inv[p], nb * 36, st));
     }
     for (int p = 0; p < 2; p++) {
-        ctx->op64.pk_link[p] = ctx->op64.pk_clov[p] = ctx->op64.pk_clov_inv[p] = nullptr;   // fp32 only
+        CLV_CHECK(dev_alloc(ctx, &ctx->op64.pk_link[p], (size_t)g.Vh * pk_link_stride(18), st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op64.pk_clov[p], (size_t)g.Vh * PK_CLOV_STRIDE, st));
+        CLV_CHECK(dev_alloc(ctx, &ctx->op64.pk_clov_inv[p], (size_t)g.Vh * PK_CLOV_STRIDE, st));
         CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_link[p], (size_t)g.Vh * pk_link_stride(ctx->op32.recon), st));
         CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov[p], (size_t)g.Vh * PK_CLOV_STRIDE, st));
         CLV_CHECK(dev_alloc(ctx, &ctx->op32.pk_clov_inv[p], (size_t)g.Vh * PK_CLOV_STRIDE, st));
@@ -395,10 +402,13 @@ int setup_operator(clover_ctx *ctx, const double *gauge_dev, cudaStream_t st)
     clover_build_kernel<<<gc, 64, 0, st>>>(g, gauge_dev, ctx->csw * ctx->kappa, ctx->op64, ctx->op32, singular);
     CLV_CUDA(cudaGetLastError());
     dim3 gp((g.Vh + 127) / 128, 16);
-    if (ctx->op32.recon == 12) pack_links_kernel<12><<<gp, 128, 0, st>>>(g, gauge_dev, ctx->op32);
-    else pack_links_kernel<18><<<gp, 128, 0, st>>>(g, gauge_dev, ctx->op32);
+    if (ctx->op32.recon == 12) pack_links_kernel<float, 12><<<gp, 128, 0, st>>>(g, gauge_dev, ctx->op32);
+    else pack_links_kernel<float, 18><<<gp, 128, 0, st>>>(g, gauge_dev, ctx->op32);
+    pack_links_kernel<double, 18><<<gp, 128, 0, st>>>(g, gauge_dev, ctx->op64);
     CLV_CUDA(cudaGetLastError());
-    pack_clover_kernel<<<dim3(((unsigned)g.Vh * 18u + 255u) / 256u, 4), 256, 0, st>>>(g, ctx->op32);
+    dim3 gk(((unsigned)g.Vh * 36u + 255u) / 256u, 4);
+    pack_clover_kernel<float><<<gk, 256, 0, st>>>(g, ctx->op32);
+    pack_clover_kernel<double><<<gk, 256, 0, st>>>(g, ctx->op64);
     CLV_CUDA(cudaGetLastError());
     int h = 0;
     CLV_CUDA(cudaMemcpyAsync(&h, singular, sizeof(int), cudaMemcpyDeviceToHost, st));
