@@ -3,7 +3,8 @@
 //   C(t0, t)  = (1/(N_r^2 scale^4)) sum_ij O_ij(t) O_ji(t0)
 // Per timeslice this is a complex GEMM  O(t) = conj(E_t) diag(gamma5) X_t^T  with M = N = N_r and K = 12 L^3 (the one dense
 // contraction of the paper's pipeline).  The propagators come out of clover_solve in fp64 and parity is asked at 1e-13, so
-// the product runs on the fp64 FMA pipe: tcgen05 has no fp64 path, and at N_r = 32 the arithmetic intensity
+// the product runs in fp64 on the tensor pipe: tcgen05 has no fp64 type, the fp64 tensor instruction is mma.sync (DMMA, same
+// peak as the FMA pipe on B200 at an eighth of the issue slots and register traffic).  At N_r = 32 the arithmetic intensity
 // (8 N_r^2 K flop over 32 N_r K bytes = N_r/4 flop/byte) sits at the fp64 ridge of a B200, not above it.
 // Canonical layouts: eta, X = [n][T][Z][Y][X][4][3] complex128; O = [T][n][n] complex128; C = [T][T] complex128.
 #include "context.h"
@@ -12,89 +13,100 @@
 
 namespace clv {
 
-constexpr int CT_TILE = 32;    // (i, j) tile edge
-constexpr int CT_KT = 16;      // k elements staged per step
-constexpr int CT_THREADS = 64;  // 8 x 8 threads, each a 4 x 4 block of outputs {ti + 8a} x {tj + 8b}
-#ifndef CT_MINB
-#define CT_MINB 8
+constexpr int CT_TILE = 32;    // (i, j) tile edge: one warp holds the whole 32 x 32 complex tile in DMMA accumulators
+constexpr int CT_KT = 8;       // complex k elements a warp stages per step (128 contiguous bytes of every row)
+constexpr int CT_KS = CT_KT + 2;   // row stride of the shared tiles in complex numbers: 8 words mod 32, so the 4 rows of a half-warp's fragment load fall in 4 disjoint bank groups
+#ifndef CT_STAGES
+#define CT_STAGES 3
 #endif
-#ifndef CT_UNROLL
-#define CT_UNROLL 2
-#endif
-constexpr int CT_UNROLL_N = CT_UNROLL;
+constexpr int CT_THREADS = 32;  // one-warp CTAs: every warp runs its own cp.async pipeline over its own k-chunk, no CTA barrier anywhere
+
+// D (8x8, fp64) += A (8x4, row) B (4x8, col): the fp64 tensor-core instruction of sm_80+ (SASS DMMA).  Fragments per thread T:
+// a = A[T/4][T%4], b = B[T%4][T/4], c/d = C[T/4][2 (T%4) + {0,1}].
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
 
 // partial[(c*T + t)*n*n + i*n + j] = sum over k-chunk c of conj(eta_i[k]) g5(k) X_j[k]
-// Two-stage cp.async pipeline: the 16-byte copies of stage s+1 (global -> shared, no registers) are in flight while stage s
-// is multiplied.  Shared tiles are stored [row][k] with a row stride of 17 x 16 bytes: the copies are coalesced along k
-// (a half-warp moves 256 contiguous bytes of one row) and the compute-phase reads of 8 different rows at one k fall in 8
-// different bank groups (lanes sharing ti get a broadcast).  conj() and the gamma5 sign are applied when the tile is read back from shared memory.
-__global__ void __launch_bounds__(CT_THREADS, CT_MINB) contract_kernel(const double2 *__restrict__ eta, const double2 *__restrict__ xs, int n, int T,
-                                                                 long K, long kchunk, int tiles, double2 *__restrict__ partial)
+// The complex product is two REAL GEMMs over the 2K interleaved (re, im) reals k' of a row:
+//   O_re = sum_k' E[i][k'] X[j][k'],   O_im = sum_k' E[i][k'] Xs[j][k'],   Xs[k'] = +X[k'+1] (k' even: the imaginary part), -X[k'-1] (k' odd)
+// (conj(e) x = (er xr + ei xi) + i (er xi - ei xr)), with the gamma5 sign of k folded into both X operands.  Operands are staged
+// [row][k] in shared memory by a CT_STAGES-deep cp.async pipeline private to the warp (16-byte copies, 128 contiguous bytes per row)
+// and read back as DMMA fragments.
+__global__ void __launch_bounds__(CT_THREADS) contract_kernel(const double2 *__restrict__ eta, const double2 *__restrict__ xs, int n, int T,
+                                                           long K, long kchunk, int tiles, double2 *__restrict__ partial)
 {
-    __shared__ __align__(16) double2 As[2][CT_TILE][CT_KT + 1], Bs[2][CT_TILE][CT_KT + 1];
+    __shared__ __align__(16) double2 As[CT_STAGES][CT_TILE][CT_KS], Bs[CT_STAGES][CT_TILE][CT_KS];
     const int c = blockIdx.x, t = blockIdx.y, bi = blockIdx.z / tiles, bj = blockIdx.z % tiles;
-    const int ti = threadIdx.x >> 3, tj = threadIdx.x & 7;
+    const int lane = threadIdx.x, fr = lane >> 2, fk = lane & 3;
     const long k0 = (long)c * kchunk, k1 = min(K, k0 + kchunk);
-    double2 acc[4][4];
+    double acc_re[4][4][2], acc_im[4][4][2];
 #pragma unroll
     for (int a = 0; a < 4; a++)
 #pragma unroll
-        for (int b = 0; b < 4; b++) acc[a][b] = make_double2(0., 0.);
+        for (int b = 0; b < 4; b++) acc_re[a][b][0] = acc_re[a][b][1] = acc_im[a][b][0] = acc_im[a][b][1] = 0.0;
 
-    auto issue = [&](int stage, long kb) {
-        // 32 rows x 16 k per operand; a half-warp copies 256 contiguous bytes of one row (coalesced), 8 copies per thread
+    auto issue = [&](int stage, long kb) {   // 32 rows x 8 k per operand: 8 lanes copy the 128 contiguous bytes of one row
+        if (kb < k1) {
 #pragma unroll
-        for (int it = 0; it < 8; it++) {
-            const int item = threadIdx.x + CT_THREADS * it, row = item >> 4, kq = item & 15;
-            const long k = kb + kq;
-            const int i = bi * CT_TILE + row, j = bj * CT_TILE + row;
-            double2 *da = &As[stage][row][kq], *db = &Bs[stage][row][kq];
-            if (k < k1 && i < n) __pipeline_memcpy_async(da, eta + ((long)i * T + t) * K + k, 16);
-            else *da = make_double2(0., 0.);
-            if (k < k1 && j < n) __pipeline_memcpy_async(db, xs + ((long)j * T + t) * K + k, 16);
-            else *db = make_double2(0., 0.);
+            for (int it = 0; it < CT_TILE * CT_KT / 32; it++) {
+                const int item = lane + 32 * it, row = item / CT_KT, kq = item % CT_KT;
+                const long k = kb + kq;
+                const int i = bi * CT_TILE + row, j = bj * CT_TILE + row;
+                double2 *da = &As[stage][row][kq], *db = &Bs[stage][row][kq];
+                if (k < k1 && i < n) __pipeline_memcpy_async(da, eta + ((long)i * T + t) * K + k, 16);
+                else *da = make_double2(0., 0.);
+                if (k < k1 && j < n) __pipeline_memcpy_async(db, xs + ((long)j * T + t) * K + k, 16);
+                else *db = make_double2(0., 0.);
+            }
         }
-        __pipeline_commit();
+        __pipeline_commit();   // (an empty group past the end keeps the wait counts uniform)
     };
 
-    issue(0, k0);
-    int stage = 0;
-    for (long kb = k0; kb < k1; kb += CT_KT, stage ^= 1) {
-        if (kb + CT_KT < k1) {
-            issue(stage ^ 1, kb + CT_KT);
-            __pipeline_wait_prior(1);
-        } else __pipeline_wait_prior(0);
-        __syncthreads();
-#pragma unroll CT_UNROLL_N
-        for (int kk = 0; kk < CT_KT; kk++) {
-            const double sgn = (((kb + kk) % 12) < 6) ? 1.0 : -1.0;   // gamma5 = diag(+,+,-,-), spin = (k % 12) / 3
-            double2 a[4], b[4];
+#pragma unroll
+    for (int s = 0; s < CT_STAGES - 1; s++) issue(s, k0 + (long)s * CT_KT);
+    int stage = 0, kbm = (int)(k0 % 12);   // kb mod 12, kept in 32-bit arithmetic (spin-colour index of the block's first element)
+    for (long kb = k0; kb < k1; kb += CT_KT, kbm = (kbm + CT_KT) % 12) {
+        issue((stage + CT_STAGES - 1) % CT_STAGES, kb + (long)(CT_STAGES - 1) * CT_KT);
+        __pipeline_wait_prior(CT_STAGES - 1);
+        __syncwarp();
+#pragma unroll
+        for (int s = 0; s < CT_KT / 2; s++) {   // four real k' (two complex) per DMMA step
+            const int kc = 2 * s + (fk >> 1), part = fk & 1;   // this lane's k' = 2 kc + part
+            const int sc = kbm + kc;                                  // < 20
+            const double sgn = (sc < 6 || (sc >= 12 && sc < 18)) ? 1.0 : -1.0;   // gamma5 = diag(+,+,-,-), spin = (k % 12) / 3
+            const double sgs = part ? -sgn : sgn;
+            double a[4], br[4], bs[4];
 #pragma unroll
             for (int r = 0; r < 4; r++) {
-                const double2 e = As[stage][ti + 8 * r][kk];
-                a[r] = make_double2(sgn * e.x, -sgn * e.y);          // conj(eta) gamma5
-                b[r] = Bs[stage][tj + 8 * r][kk];
+                const double *pa = reinterpret_cast<const double *>(&As[stage][8 * r + fr][kc]);
+                const double *pb = reinterpret_cast<const double *>(&Bs[stage][8 * r + fr][kc]);
+                a[r] = pa[part];
+                br[r] = sgn * pb[part];
+                bs[r] = sgs * pb[part ^ 1];
             }
 #pragma unroll
             for (int x = 0; x < 4; x++)
 #pragma unroll
                 for (int y = 0; y < 4; y++) {
-                    acc[x][y].x += a[x].x * b[y].x;
-                    acc[x][y].x -= a[x].y * b[y].y;
-                    acc[x][y].y += a[x].x * b[y].y;
-                    acc[x][y].y += a[x].y * b[y].x;
+                    dmma884(acc_re[x][y], a[x], br[y]);
+                    dmma884(acc_im[x][y], a[x], bs[y]);
                 }
         }
-        __syncthreads();
+        __syncwarp();   // the stage is read: it may be refilled by the next issue
+        stage = (stage + 1) % CT_STAGES;
     }
     double2 *out = partial + ((long)c * T + t) * n * n;
 #pragma unroll
-    for (int a = 0; a < 4; a++)
+    for (int x = 0; x < 4; x++)
 #pragma unroll
-        for (int b = 0; b < 4; b++) {
-            const int i = bi * CT_TILE + ti + 8 * a, j = bj * CT_TILE + tj + 8 * b;
-            if (i < n && j < n) out[(long)i * n + j] = acc[a][b];
-        }
+        for (int y = 0; y < 4; y++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const int i = bi * CT_TILE + 8 * x + fr, j = bj * CT_TILE + 8 * y + 2 * fk + e;
+                if (i < n && j < n) out[(long)i * n + j] = make_double2(acc_re[x][y][e], acc_im[x][y][e]);
+            }
 }
 
 // O[idx] = sum_c partial[c][idx], fixed order (deterministic)
@@ -139,9 +151,9 @@ int launch_contract(const double *eta, const double *xs, const int dims[4], int 
     const int T = dims[3];
     const long K = 12L * dims[0] * dims[1] * dims[2];
     const int tiles = (n + CT_TILE - 1) / CT_TILE;
-    // enough k-chunks for ~16 CTAs of 64 threads per SM, each chunk a multiple of the staging width
-    long nch = std::max<long>(1, (16L * 148 + (long)T * tiles * tiles - 1) / ((long)T * tiles * tiles));
-    nch = std::min<long>(nch, std::max<long>(1, K / (8 * CT_KT)));
+    // enough k-chunks for two waves of the one-warp CTAs resident on the device (7-11 per SM), each chunk a multiple of the staging width
+    long nch = std::max<long>(1, (20L * 148 + (long)T * tiles * tiles - 1) / ((long)T * tiles * tiles));
+    nch = std::min<long>(nch, std::max<long>(1, K / (16 * CT_KT)));
     long kchunk = (K + nch - 1) / nch;
     kchunk = (kchunk + CT_KT - 1) / CT_KT * CT_KT;
     nch = (K + kchunk - 1) / kchunk;

@@ -4,71 +4,90 @@
 // i.e. C[m][n] = norm * sum_k A[k][m] conj(B[k][n]) with A[k] = X_k (the whole canonical spinor, M = 12 V contiguous),
 // B[k] = eta_k restricted to timeslice t0 (N = 12 L^3 contiguous), K = N_r: a complex rank-N_r update whose 16-byte outputs are
 // written once.  The dagger version C'[n][m] = conj(C[m][n]) = norm * sum_k B[k][n] conj(A[k][m]) is the same kernel with the
-// operands swapped, so its stores are coalesced as well.  fp64 throughout (the propagators are fp64; parity 1e-13).
+// operands swapped, so its stores are coalesced as well.  fp64 throughout (the propagators are fp64; parity 1e-13), on the fp64
+// tensor pipe (mma.sync m8n8k4, SASS DMMA: tcgen05 has no fp64 type).
 // The paper accumulates one source at a time (a rank-1 update of the 9.7 GB array per source at L = 8: 100.8 s CPU, 8.8 s GPU,
 // Table II); here all N_r sources go through one pass, so the array is written once.
 #include "context.h"
+#include <cuda_pipeline.h>
 
 namespace clv {
 
-constexpr int FL_TILE = 64;     // outputs per CTA: 64 x 64
-constexpr int FL_KT = 8;        // sources staged per step
-constexpr int FL_THREADS = 256; // 16 x 16 threads, 4 x 4 outputs each at {ti + 16 a} x {tj + 16 b}
+constexpr int FL_TILE = 64;     // outputs per CTA: 64 x 64 complex, one 32 x 32 quadrant per warp
+constexpr int FL_KT = 32;       // sources staged per step (all of them at the paper's N_r <= 32)
+constexpr int FL_LD = FL_TILE + 4;   // row stride of the shared tiles in complex numbers (16 words mod 32: the two k rows of a fragment load fall in disjoint banks)
+constexpr int FL_THREADS = 128;
 
-// C[m*ldc + n] = norm * sum_k A[k*lda + m] * conj(B[k*ldb + n]),  m < M, n < N
-__global__ void __launch_bounds__(FL_THREADS, 2) fill_gemm_kernel(const double2 *__restrict__ A, long lda, const double2 *__restrict__ B, long ldb, int K,
+// D (8x8, fp64) += A (8x4, row) B (4x8, col) on the fp64 tensor pipe (SASS DMMA); fragments per thread T: a = A[T/4][T%4], b = B[T%4][T/4],
+// c/d = C[T/4][2 (T%4) + {0,1}]
+__device__ __forceinline__ void fill_dmma884(double (&c)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+// C[m*ldc + n] = norm * sum_k A[k*lda + m] * conj(B[k*ldb + n]),  m < M, n < N.
+// Two real GEMMs over the 2K interleaved reals k' = 2k + part of the sources:  with a = (ar, ai) and b = (br, bi),
+//   C_re = sum_k' a[k'] b[k'],   C_im = sum_k' a[k'] bs[k'],   bs[2k] = -bi, bs[2k+1] = +br      (a conj(b) = (ar br + ai bi) + i (ai br - ar bi)).
+__global__ void __launch_bounds__(FL_THREADS, 3) fill_gemm_kernel(const double2 *__restrict__ A, long lda, const double2 *__restrict__ B, long ldb, int K,
                                                                 long M, long N, double norm, double2 *__restrict__ C, long ldc)
 {
-    __shared__ __align__(16) double2 As[FL_KT][FL_TILE], Bs[FL_KT][FL_TILE];
+    extern __shared__ __align__(16) double2 fl_smem[];
+    double2(*As)[FL_LD] = reinterpret_cast<double2(*)[FL_LD]>(fl_smem);
+    double2(*Bs)[FL_LD] = reinterpret_cast<double2(*)[FL_LD]>(fl_smem + FL_KT * FL_LD);
     const long m0 = (long)blockIdx.y * FL_TILE, n0 = (long)blockIdx.x * FL_TILE;
-    const int ti = threadIdx.x >> 4, tj = threadIdx.x & 15;
-    double2 acc[4][4];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31, fr = lane >> 2, fk = lane & 3;
+    const int wm = 32 * (w >> 1), wn = 32 * (w & 1);   // this warp's quadrant
+    double acc_re[4][4][2], acc_im[4][4][2];
 #pragma unroll
     for (int a = 0; a < 4; a++)
 #pragma unroll
-        for (int b = 0; b < 4; b++) acc[a][b] = make_double2(0., 0.);
+        for (int b = 0; b < 4; b++) acc_re[a][b][0] = acc_re[a][b][1] = acc_im[a][b][0] = acc_im[a][b][1] = 0.0;
     for (int kb = 0; kb < K; kb += FL_KT) {
-        // 8 x 64 elements per operand, 2 + 2 per thread; a warp reads 512 contiguous bytes of one source
-#pragma unroll
-        for (int it = 0; it < 2; it++) {
+        // 32 x 64 elements per operand, 16-byte async copies; a warp copies 512 contiguous bytes of one source
+#pragma unroll 4
+        for (int it = 0; it < FL_KT * FL_TILE / FL_THREADS; it++) {
             const int item = threadIdx.x + FL_THREADS * it, kk = item >> 6, col = item & 63;
-            double2 a = make_double2(0., 0.), b = make_double2(0., 0.);
-            if (kb + kk < K) {
-                if (m0 + col < M) a = __ldg(A + (long)(kb + kk) * lda + m0 + col);
-                if (n0 + col < N) b = __ldg(B + (long)(kb + kk) * ldb + n0 + col);
-            }
-            As[kk][col] = a;
-            Bs[kk][col] = make_double2(b.x, -b.y);   // conj
+            double2 *da = &As[kk][col], *db = &Bs[kk][col];
+            if (kb + kk < K && m0 + col < M) __pipeline_memcpy_async(da, A + (long)(kb + kk) * lda + m0 + col, 16);
+            else *da = make_double2(0., 0.);
+            if (kb + kk < K && n0 + col < N) __pipeline_memcpy_async(db, B + (long)(kb + kk) * ldb + n0 + col, 16);
+            else *db = make_double2(0., 0.);
         }
+        __pipeline_commit();
+        __pipeline_wait_prior(0);
         __syncthreads();
-#pragma unroll
-        for (int kk = 0; kk < FL_KT; kk++) {
-            double2 a[4], b[4];
+#pragma unroll 4
+        for (int s = 0; s < FL_KT / 2; s++) {   // four reals k' = two sources per DMMA step
+            const int kc = 2 * s + (fk >> 1), part = fk & 1;
+            double a[4], br[4], bs[4];
 #pragma unroll
             for (int r = 0; r < 4; r++) {
-                a[r] = As[kk][ti + 16 * r];
-                b[r] = Bs[kk][tj + 16 * r];
+                const double *pa = reinterpret_cast<const double *>(&As[kc][wm + 8 * r + fr]);
+                const double *pb = reinterpret_cast<const double *>(&Bs[kc][wn + 8 * r + fr]);
+                a[r] = pa[part];
+                br[r] = pb[part];
+                bs[r] = part ? pb[0] : -pb[1];
             }
 #pragma unroll
             for (int x = 0; x < 4; x++)
 #pragma unroll
                 for (int y = 0; y < 4; y++) {
-                    acc[x][y].x += a[x].x * b[y].x;
-                    acc[x][y].x -= a[x].y * b[y].y;
-                    acc[x][y].y += a[x].x * b[y].y;
-                    acc[x][y].y += a[x].y * b[y].x;
+                    fill_dmma884(acc_re[x][y], a[x], br[y]);
+                    fill_dmma884(acc_im[x][y], a[x], bs[y]);
                 }
         }
         __syncthreads();
     }
+    // a thread holds two neighbouring outputs (n, n + 1) of a row: 32 contiguous bytes; the 4 lanes of a row write one 128-byte line
 #pragma unroll
     for (int x = 0; x < 4; x++) {
-        const long m = m0 + ti + 16 * x;
+        const long m = m0 + wm + 8 * x + fr;
         if (m >= M) continue;
 #pragma unroll
         for (int y = 0; y < 4; y++) {
-            const long n = n0 + tj + 16 * y;
-            if (n < N) C[m * ldc + n] = make_double2(norm * acc[x][y].x, norm * acc[x][y].y);   // 16 lanes -> 256 contiguous bytes
+            const long n = n0 + wn + 8 * y + 2 * fk;
+            if (n < N) C[m * ldc + n] = make_double2(norm * acc_re[x][y][0], norm * acc_im[x][y][0]);
+            if (n + 1 < N) C[m * ldc + n + 1] = make_double2(norm * acc_re[x][y][1], norm * acc_im[x][y][1]);
         }
     }
 }
@@ -79,12 +98,15 @@ int launch_fill(const double *x, const double *eta, const int dims[4], int n, in
     const long M = 12 * V, N = 12 * V3;              // rows (t, z, a), columns (x, b)
     const double2 *A = (const double2 *)x, *B = (const double2 *)eta + (long)t0 * N;
     const double norm = 1.0 / ((double)n * scale * scale);
+    constexpr size_t smem = sizeof(double2) * 2 * FL_KT * FL_LD;
+    static const cudaError_t attr = cudaFuncSetAttribute(fill_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    CLV_CUDA(attr);
     if (!dagger) {
         dim3 grid((unsigned)((N + FL_TILE - 1) / FL_TILE), (unsigned)((M + FL_TILE - 1) / FL_TILE));
-        fill_gemm_kernel<<<grid, FL_THREADS, 0, st>>>(A, M, B, M, n, M, N, norm, (double2 *)s, N);
+        fill_gemm_kernel<<<grid, FL_THREADS, smem, st>>>(A, M, B, M, n, M, N, norm, (double2 *)s, N);
     } else {  // S^dagger[x, b, t, z, a]: rows (x, b), columns (t, z, a); operands swapped
         dim3 grid((unsigned)((M + FL_TILE - 1) / FL_TILE), (unsigned)((N + FL_TILE - 1) / FL_TILE));
-        fill_gemm_kernel<<<grid, FL_THREADS, 0, st>>>(B, M, A, M, n, N, M, norm, (double2 *)s, M);
+        fill_gemm_kernel<<<grid, FL_THREADS, smem, st>>>(B, M, A, M, n, N, M, norm, (double2 *)s, M);
     }
     CLV_CUDA(cudaGetLastError());
     return 0;
