@@ -258,8 +258,12 @@ def main():
     bytes_xrp = 24 * b * 9      # one sweep: reads x, p, s, t, r, q0, writes x, r, p
     prec = 32 if cfg["mixed"] else 64
     rt, pair = ("float" if cfg["mixed"] else "double"), (cfg["mixed"] and batch >= 2)
-    kname = (lambda what: f"dslash2_kernel<B={batch},recon={g},{what}> (fp32, one thread per site and rhs pair)") if pair else \
-            (lambda what: f"dslash_kernel<{rt},B={batch},recon={g},{what}>")
+    if cfg["mixed"] and batch == 8:
+        kname = lambda what: f"dslash3_kernel<B=8,recon={g},{what}> (fp32, persistent one-warp CTAs, one thread per site and rhs pair, operator records by cp.async.bulk)"
+    elif pair:
+        kname = lambda what: f"dslash2_kernel<B={batch},recon={g},{what}> (fp32, one thread per site and rhs pair)"
+    else:
+        kname = lambda what: f"dslash_kernel<{rt},B={batch},recon={g},{what}>"
     timed = "CUDA events around every launch inside the timed steps"
     table = {}   # name -> (kernel, launches, summed ms, algorithmic bytes / site / rhs, flop / site / rhs, traffic key)
     if kstats["n_a_minus_hop"]:
@@ -359,7 +363,7 @@ def main():
         fp64_peak = 148 * 64 * 2 * 1.965e9     # fp64 FMA lanes per SM x SMs x 2 flop x max clock
         contraction = {"what": "O_ij(t) = sum_y eta_i^* gamma5 X_j, all t, N_r = %d (paper eq. 7.6)" % n_rhs, "ms": tc * 1e3,
                        "gbs": cbytes / tc / 1e9, "frac_hbm": cbytes / tc / 1e9 / peaks["hbm_gbs"], "tflops_fp64": cflop / tc / 1e12,
-                       "frac_fp64_alu": cflop / tc / fp64_peak, "bound": "alu (fp64 FMA) ~ hbm", "dtype": "f64"}
+                       "frac_fp64_alu": cflop / tc / fp64_peak, "bound": "alu (fp64 tensor pipe, DMMA) ~ hbm", "dtype": "f64"}
         del o
 
     # ---- NEXT row (S 8(f) rank 2): outer-product fill S and S^dagger at the paper's Table II size (L = 8: 8^3x16) ----
