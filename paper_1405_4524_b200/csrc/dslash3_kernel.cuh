@@ -151,8 +151,8 @@ template <int DOT> __device__ __forceinline__ void dots_f(const cx<float> acc[12
 // Reduce-scatter of a warp tile's partial sums (B = 8, one-warp CTAs: lane = 4 site + pair, 8 sites x 4 rhs pairs).  v holds the NV = 2 ND
 // sums of this thread's two rhs, padded to 8 K values (K = 1 | 2).  Three butterfly steps over the site bits of the lane, each sending one
 // half of the values and keeping the other, leave lane (site s, pair q) with the sums over the tile's 8 sites of values K s .. K s + K - 1 of
-// pair q: 7 or 14 shuffles instead of 3 NV, and K accumulators per thread instead of NV -- the hop has no registers for more.
-// (The 8 sites of a tile are summed in fp32, tiles in fp64; fixed order: deterministic.)
+// pair q: 7 or 14 shuffles instead of 3 NV, and K values per thread to store instead of NV.
+// (The 8 sites of a tile are summed in fp32; the tiles' lines are added in fp64 by the scalar kernel in a fixed order: deterministic.)
 template <int K> __device__ __forceinline__ void reduce_scatter_sites(float (&v)[8 * K], float (&out)[K])
 {
     const unsigned lane = threadIdx.x & 31u;
@@ -190,7 +190,7 @@ template <int K> __device__ __forceinline__ void reduce_scatter_sites(float (&v)
 // slower).  Tiles are handed out in order by an atomic counter (`sched[0]`; the first gridDim.x tiles statically), not round-robin: CTAs
 // that fall behind would otherwise spread the window of sites in flight over many timeslices and the neighbour gathers would stop hitting L2
 // (measured at 32^3x64: a round-robin assignment lost everything the records had gained).  The last CTA to leave re-arms the counters for
-// the next launch.  Dot-product variants leave ONE line of partial sums per CTA for the whole launch.
+// the next launch.  Dot-product variants write one line of partial sums per tile (the sums of the tile's 8 sites).
 #ifndef CLV_R3_CBUF
 #define CLV_R3_CBUF 1
 #endif
@@ -239,7 +239,6 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
         post_links(tile, 0);
         if (CLOV) post_clover(tile, 0);
     }
-    double sum[K] = {};
     do {
         const int buf = it & 1, cbuf = NCB == 2 ? buf : 0;
         const unsigned par = (it >> 1) & 1, cpar = NCB == 2 ? par : (it & 1);
@@ -351,11 +350,21 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
                 dots_f<DOT>(accB, xB, wB, v + ND);
             }
         }
-        if (RED) {
+        if (RED) {   // one line of partial sums per TILE, indexed by the tile: the scalar kernel adds the lines in a fixed order, so the
+            // result does not depend on which CTA the scheduler gave the tile to (solves stay bit-reproducible)
             float t[K];
             reduce_scatter_sites<K>(v, t);
+            // lane (site s, pair q) holds values K s .. K s + K - 1 of pair q: value c < ND belongs to rhs 2q, else c - ND to rhs 2q + 1
+            const int s = threadIdx.x >> 2, q = threadIdx.x & 3;
 #pragma unroll
-            for (int k = 0; k < K; k++) sum[k] += (double)t[k];
+            for (int k = 0; k < K; k++) {
+                const int cidx = K * s + k;
+                if (cidx < 2 * ND) {
+                    const int r = 2 * q + (cidx >= ND), cc = cidx % ND;
+                    if (cc < 3) a.partial[((size_t)tile * B + r) * 4 + cc] = (double)t[k];
+                    else a.partial2[((size_t)tile * B + r) * 4 + (cc - 3)] = (double)t[k];
+                }
+            }
         }
         __syncthreads();   // every read of this tile's link records is done before the buffer is posted again
         tile = next_s[buf];
@@ -364,18 +373,6 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
     if (threadIdx.x == 0) {   // the last CTA to finish re-arms the tile counter for the next launch on this context
         __threadfence();
         if (atomicInc(&sched[1], gridDim.x - 1) == gridDim.x - 1) sched[0] = 0;
-    }
-    if (RED) {   // lane (site s, pair q) holds values K s .. K s + K - 1 of pair q: value c < ND belongs to rhs 2q, else c - ND to rhs 2q + 1
-        const int s = threadIdx.x >> 2, q = threadIdx.x & 3;
-#pragma unroll
-        for (int k = 0; k < K; k++) {
-            const int cidx = K * s + k;
-            if (cidx < 2 * ND) {
-                const int r = 2 * q + (cidx >= ND), cc = cidx % ND;
-                if (cc < 3) a.partial[((size_t)blockIdx.x * B + r) * 4 + cc] = sum[k];
-                else a.partial2[((size_t)blockIdx.x * B + r) * 4 + (cc - 3)] = sum[k];
-            }
-        }
     }
 }
 

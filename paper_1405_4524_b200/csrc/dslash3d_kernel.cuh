@@ -98,7 +98,6 @@ dslash3d_kernel(const Geom g, const OpData<double> op, const DslashArgs<double> 
         post_links(tile, 0);
         if (CLOV) post_clover(tile);
     }
-    double sum = 0.0;
     do {
         const int buf = it & 1;
         const unsigned par = (it >> 1) & 1, cpar = it & 1;
@@ -179,10 +178,15 @@ dslash3d_kernel(const Geom g, const OpData<double> op, const DslashArgs<double> 
                 } else if (a.out) store_spinor(a.out, j, acc);   // neither: only the norm is wanted (final verification)
             } else store_spinor(a.out, j, acc);
         }
-        if (DOT == DOT_RES) {   // sum over the tile's 4 sites (lane bits 3, 4): every lane ends with its rhs' sum; tiles accumulate in order
+        if (DOT == DOT_RES) {   // sum over the tile's 4 sites (lane bits 3, 4); one line of partial sums per TILE, indexed by the tile, so that
+            // the scalar kernel's fixed-order sum does not depend on the scheduler (bit-reproducible)
             d0 += __shfl_xor_sync(0xffffffffu, d0, 8);
             d0 += __shfl_xor_sync(0xffffffffu, d0, 16);
-            sum += d0;
+            if (threadIdx.x < B) {
+                double *o = a.partial + ((size_t)tile * B + threadIdx.x) * 4;
+                o[0] = d0;
+                o[1] = o[2] = o[3] = 0.0;
+            }
         }
         __syncthreads();   // every read of this tile's link records is done before the buffer is posted again
         tile = next_s[buf];
@@ -191,11 +195,6 @@ dslash3d_kernel(const Geom g, const OpData<double> op, const DslashArgs<double> 
     if (threadIdx.x == 0) {   // the last CTA to finish re-arms the tile counter for the next launch on this context
         __threadfence();
         if (atomicInc(&sched[1], gridDim.x - 1) == gridDim.x - 1) sched[0] = 0;
-    }
-    if (DOT == DOT_RES && threadIdx.x < B) {   // one line of partial sums per CTA for the whole launch
-        double *o = a.partial + ((size_t)blockIdx.x * B + threadIdx.x) * 4;
-        o[0] = sum;
-        o[1] = o[2] = o[3] = 0.0;
     }
 }
 

@@ -88,7 +88,7 @@ static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, con
         CLV_CUDA(attr);                                                                                                  \
         const unsigned ntiles = ((unsigned)g.Vh + (2 * BLK / B) - 1) / (2 * BLK / B);                                    \
         const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * CLV_R3_GRID_PER_SM);                           \
-        if (grid_out) *grid_out = (int)grid;                                                                             \
+        if (grid_out) *grid_out = (int)ntiles;   /* lines of partial sums: one per tile */                                \
         kern<<<grid, BLK, 0, st>>>(g, op, a, ctx->sched);                                                                \
         break;                                                                                                           \
     }
@@ -132,7 +132,7 @@ static bool launch_dslash3d(const clover_ctx *ctx, const OpData<double> &op, con
         if (attr != cudaSuccess) { set_error("cudaFuncSetAttribute failed: %s", cudaGetErrorString(attr)); *rc = CLOVER_ECUDA; return true; } \
         const unsigned ntiles = ((unsigned)g.Vh + 3) / 4;                                                                \
         const unsigned grid = std::min<unsigned>(ntiles, (unsigned)n_sm * CLV_R3D_WARPS_PER_SM);                         \
-        if (grid_out) *grid_out = (int)grid;                                                                             \
+        if (grid_out) *grid_out = (int)ntiles;   /* lines of partial sums: one per tile */                                \
         kern<<<grid, 32, 0, st>>>(g, op, a, ctx->sched);                                                                 \
         break;                                                                                                           \
     }

@@ -91,7 +91,8 @@ static int ensure_work(clover_ctx *ctx, int B, size_t real_bytes, bool staging, 
         }
         cudaFree(W->partial);
         // twice the blocks of one Dslash launch: the final verification reduces the partials of two launches (even + odd) at once
-        W->partial_blocks = 2 * std::max<int>(((unsigned)g.Vh * B + dslash_block_size() - 1) / dslash_block_size(), 148 * 8);
+        // (one line per 32 threads of a launch at most: the persistent B = 8 kernels write one line per tile of 8 or 4 sites)
+        W->partial_blocks = 2 * std::max<int>(((unsigned)g.Vh * B + 31) / 32, 148 * 8);
         CLV_CUDA(cudaMalloc(&W->partial, (size_t)W->partial_blocks * B * 4 * sizeof(double)));
         CLV_CUDA(cudaMemsetAsync(W->partial, 0, (size_t)W->partial_blocks * B * 4 * sizeof(double), st));
         cudaFree(W->partial2);

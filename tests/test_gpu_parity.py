@@ -308,3 +308,35 @@ def test_solve_at_the_papers_parameter_point(B, dims, eps):
         _, infos64, bad64 = S.ctx.solve(eta, tol=tol, batch=8, mixed=False, max_iter=5000)
         assert bad64 == 0 and infos[0]["iters"] <= 2.5 * infos64[0]["iters"] + 20, (infos[0], infos64[0])
     S.ctx.close()
+
+
+def test_persistent_b8_kernels_loop_over_tiles(B, monkeypatch):
+    """16^4 at batch 8: 4096 tiles of 8 sites for the 1776 persistent CTAs of dslash3_kernel (8192 tiles of 4 sites for the 1184 of
+    dslash3d_kernel), so every CTA loops, draws tiles from the atomic scheduler, re-posts its record buffers and carries its partial
+    sums across tiles.  Operators against the oracle element by element; then the solve in both orderings of the iteration (the
+    textbook one launches the DOT_W / DOT_X variants), mixed and fp64, bit-reproducible, against the oracle's D."""
+    dims = (16, 16, 16, 16)
+    S = Setup(B, dims, 0.4, 0.118, 1.5, seed=55)
+    psi = wl.random_spinor(dims, 56, 8)
+    for op in (B.OP_HOP_FULL, B.OP_D_FULL, B.OP_MHAT):
+        want = np.stack([S.ref(B, op, psi[r]) for r in range(8)])
+        assert nerr(S.ctx.dslash_apply(op, dev(psi)).cpu().numpy(), want) < 1e-13, op
+        assert nerr(S.ctx.dslash_apply(op, dev(psi.astype(np.complex64))).cpu().numpy(), want) < 1e-6, op
+    eta = B.noise_fill(dims, 57, 8, scale=wl.INV_SQRT2)
+    e = eta.cpu().numpy()
+    sols = {}
+    for merged in ("1", "0"):
+        monkeypatch.setenv("CLOVER_MERGED", merged)
+        for mixed in (True, False):
+            psi1, infos1, bad1 = S.ctx.solve(eta, tol=wl.TOL, batch=8, mixed=mixed)
+            psi2, infos2, bad2 = S.ctx.solve(eta, tol=wl.TOL, batch=8, mixed=mixed)
+            assert bad1 == bad2 == 0 and torch.equal(psi1, psi2) and infos1 == infos2, (merged, mixed)
+            sols[(merged, mixed)] = psi1.cpu().numpy()
+            for r in (0, 7):
+                res = np.linalg.norm(e[r] - oracle.apply_D(S.U, S.A, S.bc, S.kappa, sols[(merged, mixed)][r])) / np.linalg.norm(e[r])
+                assert res <= wl.TOL and abs(infos1[r]["true_resid"] - res) <= 1e-3 * res + 1e-14, (merged, mixed, r, res)
+    want, oi = oracle.bicgstab(S.U, S.A, S.bc, S.kappa, e[3], tol=1e-12)
+    assert oi["status"] == 0
+    for k, p in sols.items():
+        assert np.linalg.norm(p[3] - want) / np.linalg.norm(want) < 1e-8, k
+    S.ctx.close()
