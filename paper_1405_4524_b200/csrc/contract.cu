@@ -13,13 +13,11 @@
 
 namespace clv {
 
-constexpr int CT_TILE = 32;    // (i, j) tile edge: one warp holds the whole 32 x 32 complex tile in DMMA accumulators
-constexpr int CT_KT = 8;       // complex k elements a warp stages per step (128 contiguous bytes of every row)
-constexpr int CT_KS = CT_KT + 2;   // row stride of the shared tiles in complex numbers: 8 words mod 32, so the 4 rows of a half-warp's fragment load fall in 4 disjoint bank groups
-#ifndef CT_STAGES
-#define CT_STAGES 3
-#endif
-constexpr int CT_THREADS = 32;  // one-warp CTAs: every warp runs its own cp.async pipeline over its own k-chunk, no CTA barrier anywhere
+constexpr int CT_TILE = 32;    // (i, j) tile edge
+constexpr int CT_KT = 16;      // complex k elements staged per step (256 contiguous bytes of every row)
+constexpr int CT_KS = CT_KT + 4;   // row stride of the shared tiles in complex numbers: 16 words mod 32, so the two rows of a quarter-warp's 16-byte fragment loads fall in disjoint banks
+constexpr int CT_WARPS = 2;    // warp w owns columns [16 w, 16 w + 16) of the tile: 4 x 2 DMMA tiles x 3 accumulator sets
+constexpr int CT_THREADS = 32 * CT_WARPS;
 
 // D (8x8, fp64) += A (8x4, row) B (4x8, col): the fp64 tensor-core instruction of sm_80+ (SASS DMMA).  Fragments per thread T:
 // a = A[T/4][T%4], b = B[T%4][T/4], c/d = C[T/4][2 (T%4) + {0,1}].
@@ -29,83 +27,85 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b)
 }
 
 // partial[(c*T + t)*n*n + i*n + j] = sum over k-chunk c of conj(eta_i[k]) g5(k) X_j[k]
-// The complex product is two REAL GEMMs over the 2K interleaved (re, im) reals k' of a row:
-//   O_re = sum_k' E[i][k'] X[j][k'],   O_im = sum_k' E[i][k'] Xs[j][k'],   Xs[k'] = +X[k'+1] (k' even: the imaginary part), -X[k'-1] (k' odd)
-// (conj(e) x = (er xr + ei xi) + i (er xi - ei xr)), with the gamma5 sign of k folded into both X operands.  Operands are staged
-// [row][k] in shared memory by a CT_STAGES-deep cp.async pipeline private to the warp (16-byte copies, 128 contiguous bytes per row)
-// and read back as DMMA fragments.
+// Three REAL GEMMs per complex one (Gauss' three-multiplication form, a quarter fewer DMMA than the four-product form): with e = a + i b,
+// g5 x = c + i d,   conj(e) x = (ac + bd) + i (ad - bc) = (k1 + k3) + i (k1 + k2),   k1 = (a - b) c,  k2 = a (d - c),  k3 = b (c + d);
+// the three sums over k are kept in three accumulator sets and combined once at the end.  Operands are staged [row][k] in shared memory by a
+// two-stage cp.async pipeline (16-byte copies, coalesced along k); a 16-byte fragment load brings (a, b) or (c, d) of one (row, k).
 __global__ void __launch_bounds__(CT_THREADS) contract_kernel(const double2 *__restrict__ eta, const double2 *__restrict__ xs, int n, int T,
                                                            long K, long kchunk, int tiles, double2 *__restrict__ partial)
 {
-    __shared__ __align__(16) double2 As[CT_STAGES][CT_TILE][CT_KS], Bs[CT_STAGES][CT_TILE][CT_KS];
+    __shared__ __align__(16) double2 As[2][CT_TILE][CT_KS], Bs[2][CT_TILE][CT_KS];
     const int c = blockIdx.x, t = blockIdx.y, bi = blockIdx.z / tiles, bj = blockIdx.z % tiles;
-    const int lane = threadIdx.x, fr = lane >> 2, fk = lane & 3;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31, fr = lane >> 2, fk = lane & 3;
     const long k0 = (long)c * kchunk, k1 = min(K, k0 + kchunk);
-    double acc_re[4][4][2], acc_im[4][4][2];
+    double acc1[4][2][2], acc2[4][2][2], acc3[4][2][2];
 #pragma unroll
-    for (int a = 0; a < 4; a++)
+    for (int x = 0; x < 4; x++)
 #pragma unroll
-        for (int b = 0; b < 4; b++) acc_re[a][b][0] = acc_re[a][b][1] = acc_im[a][b][0] = acc_im[a][b][1] = 0.0;
+        for (int y = 0; y < 2; y++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) acc1[x][y][e] = acc2[x][y][e] = acc3[x][y][e] = 0.0;
 
-    auto issue = [&](int stage, long kb) {   // 32 rows x 8 k per operand: 8 lanes copy the 128 contiguous bytes of one row
-        if (kb < k1) {
+    auto issue = [&](int stage, long kb) {   // 32 rows x 16 k per operand: 16 lanes copy the 256 contiguous bytes of one row
 #pragma unroll
-            for (int it = 0; it < CT_TILE * CT_KT / 32; it++) {
-                const int item = lane + 32 * it, row = item / CT_KT, kq = item % CT_KT;
-                const long k = kb + kq;
-                const int i = bi * CT_TILE + row, j = bj * CT_TILE + row;
-                double2 *da = &As[stage][row][kq], *db = &Bs[stage][row][kq];
-                if (k < k1 && i < n) __pipeline_memcpy_async(da, eta + ((long)i * T + t) * K + k, 16);
-                else *da = make_double2(0., 0.);
-                if (k < k1 && j < n) __pipeline_memcpy_async(db, xs + ((long)j * T + t) * K + k, 16);
-                else *db = make_double2(0., 0.);
-            }
+        for (int it = 0; it < CT_TILE * CT_KT / CT_THREADS; it++) {
+            const int item = threadIdx.x + CT_THREADS * it, row = item / CT_KT, kq = item % CT_KT;
+            const long k = kb + kq;
+            const int i = bi * CT_TILE + row, j = bj * CT_TILE + row;
+            double2 *da = &As[stage][row][kq], *db = &Bs[stage][row][kq];
+            if (k < k1 && i < n) __pipeline_memcpy_async(da, eta + ((long)i * T + t) * K + k, 16);
+            else *da = make_double2(0., 0.);
+            if (k < k1 && j < n) __pipeline_memcpy_async(db, xs + ((long)j * T + t) * K + k, 16);
+            else *db = make_double2(0., 0.);
         }
-        __pipeline_commit();   // (an empty group past the end keeps the wait counts uniform)
+        __pipeline_commit();
     };
 
-#pragma unroll
-    for (int s = 0; s < CT_STAGES - 1; s++) issue(s, k0 + (long)s * CT_KT);
+    issue(0, k0);
     int stage = 0, kbm = (int)(k0 % 12);   // kb mod 12, kept in 32-bit arithmetic (spin-colour index of the block's first element)
-    for (long kb = k0; kb < k1; kb += CT_KT, kbm = (kbm + CT_KT) % 12) {
-        issue((stage + CT_STAGES - 1) % CT_STAGES, kb + (long)(CT_STAGES - 1) * CT_KT);
-        __pipeline_wait_prior(CT_STAGES - 1);
-        __syncwarp();
+    for (long kb = k0; kb < k1; kb += CT_KT, stage ^= 1, kbm = (kbm + CT_KT) % 12) {
+        if (kb + CT_KT < k1) {
+            issue(stage ^ 1, kb + CT_KT);
+            __pipeline_wait_prior(1);
+        } else __pipeline_wait_prior(0);
+        __syncthreads();
 #pragma unroll
-        for (int s = 0; s < CT_KT / 2; s++) {   // four real k' (two complex) per DMMA step
-            const int kc = 2 * s + (fk >> 1), part = fk & 1;   // this lane's k' = 2 kc + part
-            const int sc = kbm + kc;                                  // < 20
-            const double sgn = (sc < 6 || (sc >= 12 && sc < 18)) ? 1.0 : -1.0;   // gamma5 = diag(+,+,-,-), spin = (k % 12) / 3
-            const double sgs = part ? -sgn : sgn;
-            double a[4], br[4], bs[4];
+        for (int s = 0; s < CT_KT / 4; s++) {   // four complex k per DMMA step; this lane's k = 4 s + fk
+            const int sc = kbm + 4 * s + fk;                                     // < 28
+            const int scm = sc >= 24 ? sc - 24 : (sc >= 12 ? sc - 12 : sc);
+            const double sgn = scm < 6 ? 1.0 : -1.0;                             // gamma5 = diag(+,+,-,-), spin = (k % 12) / 3
+            double a[4], b[4], amb[4], cc[2], dmc[2], cpd[2];
 #pragma unroll
             for (int r = 0; r < 4; r++) {
-                const double *pa = reinterpret_cast<const double *>(&As[stage][8 * r + fr][kc]);
-                const double *pb = reinterpret_cast<const double *>(&Bs[stage][8 * r + fr][kc]);
-                a[r] = pa[part];
-                br[r] = sgn * pb[part];
-                bs[r] = sgs * pb[part ^ 1];
+                const double2 e = As[stage][8 * r + fr][4 * s + fk];
+                a[r] = e.x; b[r] = e.y; amb[r] = e.x - e.y;
+            }
+#pragma unroll
+            for (int r = 0; r < 2; r++) {
+                const double2 x = Bs[stage][16 * w + 8 * r + fr][4 * s + fk];
+                const double xc = sgn * x.x, xd = sgn * x.y;
+                cc[r] = xc; dmc[r] = xd - xc; cpd[r] = xc + xd;
             }
 #pragma unroll
             for (int x = 0; x < 4; x++)
 #pragma unroll
-                for (int y = 0; y < 4; y++) {
-                    dmma884(acc_re[x][y], a[x], br[y]);
-                    dmma884(acc_im[x][y], a[x], bs[y]);
+                for (int y = 0; y < 2; y++) {
+                    dmma884(acc1[x][y], amb[x], cc[y]);
+                    dmma884(acc2[x][y], a[x], dmc[y]);
+                    dmma884(acc3[x][y], b[x], cpd[y]);
                 }
         }
-        __syncwarp();   // the stage is read: it may be refilled by the next issue
-        stage = (stage + 1) % CT_STAGES;
+        __syncthreads();
     }
     double2 *out = partial + ((long)c * T + t) * n * n;
 #pragma unroll
     for (int x = 0; x < 4; x++)
 #pragma unroll
-        for (int y = 0; y < 4; y++)
+        for (int y = 0; y < 2; y++)
 #pragma unroll
             for (int e = 0; e < 2; e++) {
-                const int i = bi * CT_TILE + 8 * x + fr, j = bj * CT_TILE + 8 * y + 2 * fk + e;
-                if (i < n && j < n) out[(long)i * n + j] = make_double2(acc_re[x][y][e], acc_im[x][y][e]);
+                const int i = bi * CT_TILE + 8 * x + fr, j = bj * CT_TILE + 16 * w + 8 * y + 2 * fk + e;
+                if (i < n && j < n) out[(long)i * n + j] = make_double2(acc1[x][y][e] + acc3[x][y][e], acc1[x][y][e] + acc2[x][y][e]);
             }
 }
 
@@ -151,9 +151,9 @@ int launch_contract(const double *eta, const double *xs, const int dims[4], int 
     const int T = dims[3];
     const long K = 12L * dims[0] * dims[1] * dims[2];
     const int tiles = (n + CT_TILE - 1) / CT_TILE;
-    // enough k-chunks for two waves of the one-warp CTAs resident on the device (7-11 per SM), each chunk a multiple of the staging width
-    long nch = std::max<long>(1, (20L * 148 + (long)T * tiles * tiles - 1) / ((long)T * tiles * tiles));
-    nch = std::min<long>(nch, std::max<long>(1, K / (16 * CT_KT)));
+    // enough k-chunks for two waves of the CTAs resident on the device (5 per SM), each chunk a multiple of the staging width
+    long nch = std::max<long>(1, (10L * 148 + (long)T * tiles * tiles - 1) / ((long)T * tiles * tiles));
+    nch = std::min<long>(nch, std::max<long>(1, K / (8 * CT_KT)));
     long kchunk = (K + nch - 1) / nch;
     kchunk = (kchunk + CT_KT - 1) / CT_KT * CT_KT;
     nch = (K + kchunk - 1) / kchunk;
