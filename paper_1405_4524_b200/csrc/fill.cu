@@ -13,9 +13,9 @@
 
 namespace clv {
 
-constexpr int FL_TILE = 64;     // outputs per CTA: 64 x 64 complex, one 32 x 32 quadrant per warp
+constexpr int FL_TILE = 64;     // outputs per CTA: 64 x 64 complex, one 32 x 32 quadrant per warp (computed as two 32 x 16 halves)
 constexpr int FL_KT = 32;       // sources staged per step (all of them at the paper's N_r <= 32)
-constexpr int FL_LD = FL_TILE + 4;   // row stride of the shared tiles in complex numbers (16 words mod 32: the two k rows of a fragment load fall in disjoint banks)
+constexpr int FL_LD = FL_TILE + 2;   // row stride of the shared tiles in complex numbers (8 words mod 32: the four source rows x two columns of a quarter-warp's 16-byte fragment loads fall in disjoint banks)
 constexpr int FL_THREADS = 128;
 
 // D (8x8, fp64) += A (8x4, row) B (4x8, col) on the fp64 tensor pipe (SASS DMMA); fragments per thread T: a = A[T/4][T%4], b = B[T%4][T/4],
@@ -26,8 +26,9 @@ __device__ __forceinline__ void fill_dmma884(double (&c)[2], double a, double b)
 }
 
 // C[m*ldc + n] = norm * sum_k A[k*lda + m] * conj(B[k*ldb + n]),  m < M, n < N.
-// Two real GEMMs over the 2K interleaved reals k' = 2k + part of the sources:  with a = (ar, ai) and b = (br, bi),
-//   C_re = sum_k' a[k'] b[k'],   C_im = sum_k' a[k'] bs[k'],   bs[2k] = -bi, bs[2k+1] = +br      (a conj(b) = (ar br + ai bi) + i (ai br - ar bi)).
+// Three REAL GEMMs over the sources per complex one (Gauss' three-multiplication form: a quarter fewer DMMA than four products).  With
+// a = ar + i ai, b = br + i bi:   a conj(b) = (ar br + ai bi) + i (ai br - ar bi) = (k1 - k3) + i (k1 + k2),
+//   k1 = (ar + ai) br,   k2 = ar (-bi - br),   k3 = ai (br - bi);   the three sums over k sit in three accumulator sets, combined at the end.
 __global__ void __launch_bounds__(FL_THREADS, 3) fill_gemm_kernel(const double2 *__restrict__ A, long lda, const double2 *__restrict__ B, long ldb, int K,
                                                                 long M, long N, double norm, double2 *__restrict__ C, long ldc)
 {
@@ -37,57 +38,66 @@ __global__ void __launch_bounds__(FL_THREADS, 3) fill_gemm_kernel(const double2 
     const long m0 = (long)blockIdx.y * FL_TILE, n0 = (long)blockIdx.x * FL_TILE;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31, fr = lane >> 2, fk = lane & 3;
     const int wm = 32 * (w >> 1), wn = 32 * (w & 1);   // this warp's quadrant
-    double acc_re[4][4][2], acc_im[4][4][2];
+    const bool single = K <= FL_KT;                    // the paper's case: every source staged at once, the two halves share the staging
+    for (int half = 0; half < 2; half++) {             // columns [wn + 16 half, wn + 16 half + 16) of the quadrant
+        double acc1[4][2][2], acc2[4][2][2], acc3[4][2][2];
 #pragma unroll
-    for (int a = 0; a < 4; a++)
+        for (int x = 0; x < 4; x++)
 #pragma unroll
-        for (int b = 0; b < 4; b++) acc_re[a][b][0] = acc_re[a][b][1] = acc_im[a][b][0] = acc_im[a][b][1] = 0.0;
-    for (int kb = 0; kb < K; kb += FL_KT) {
-        // 32 x 64 elements per operand, 16-byte async copies; a warp copies 512 contiguous bytes of one source
+            for (int y = 0; y < 2; y++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) acc1[x][y][e] = acc2[x][y][e] = acc3[x][y][e] = 0.0;
+        for (int kb = 0; kb < K; kb += FL_KT) {
+            if (!(single && half == 1)) {
+                if (half == 1 || kb > 0) __syncthreads();   // the previous block has been read
+                // 32 x 64 elements per operand, 16-byte async copies; a warp copies 512 contiguous bytes of one source
 #pragma unroll 4
-        for (int it = 0; it < FL_KT * FL_TILE / FL_THREADS; it++) {
-            const int item = threadIdx.x + FL_THREADS * it, kk = item >> 6, col = item & 63;
-            double2 *da = &As[kk][col], *db = &Bs[kk][col];
-            if (kb + kk < K && m0 + col < M) __pipeline_memcpy_async(da, A + (long)(kb + kk) * lda + m0 + col, 16);
-            else *da = make_double2(0., 0.);
-            if (kb + kk < K && n0 + col < N) __pipeline_memcpy_async(db, B + (long)(kb + kk) * ldb + n0 + col, 16);
-            else *db = make_double2(0., 0.);
-        }
-        __pipeline_commit();
-        __pipeline_wait_prior(0);
-        __syncthreads();
-#pragma unroll 4
-        for (int s = 0; s < FL_KT / 2; s++) {   // four reals k' = two sources per DMMA step
-            const int kc = 2 * s + (fk >> 1), part = fk & 1;
-            double a[4], br[4], bs[4];
-#pragma unroll
-            for (int r = 0; r < 4; r++) {
-                const double *pa = reinterpret_cast<const double *>(&As[kc][wm + 8 * r + fr]);
-                const double *pb = reinterpret_cast<const double *>(&Bs[kc][wn + 8 * r + fr]);
-                a[r] = pa[part];
-                br[r] = pb[part];
-                bs[r] = part ? pb[0] : -pb[1];
-            }
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 4; y++) {
-                    fill_dmma884(acc_re[x][y], a[x], br[y]);
-                    fill_dmma884(acc_im[x][y], a[x], bs[y]);
+                for (int it = 0; it < FL_KT * FL_TILE / FL_THREADS; it++) {
+                    const int item = threadIdx.x + FL_THREADS * it, kk = item >> 6, col = item & 63;
+                    double2 *da = &As[kk][col], *db = &Bs[kk][col];
+                    if (kb + kk < K && m0 + col < M) __pipeline_memcpy_async(da, A + (long)(kb + kk) * lda + m0 + col, 16);
+                    else *da = make_double2(0., 0.);
+                    if (kb + kk < K && n0 + col < N) __pipeline_memcpy_async(db, B + (long)(kb + kk) * ldb + n0 + col, 16);
+                    else *db = make_double2(0., 0.);
                 }
+                __pipeline_commit();
+                __pipeline_wait_prior(0);
+                __syncthreads();
+            }
+#pragma unroll 2
+            for (int s = 0; s < FL_KT / 4; s++) {   // four sources per DMMA step; this lane's source = 4 s + fk
+                double ar[4], ai[4], apq[4], br[2], bm[2], bp[2];
+#pragma unroll
+                for (int r = 0; r < 4; r++) {
+                    const double2 a = As[4 * s + fk][wm + 8 * r + fr];
+                    ar[r] = a.x; ai[r] = a.y; apq[r] = a.x + a.y;
+                }
+#pragma unroll
+                for (int r = 0; r < 2; r++) {
+                    const double2 b = Bs[4 * s + fk][wn + 16 * half + 8 * r + fr];
+                    br[r] = b.x; bm[r] = -b.y - b.x; bp[r] = b.x - b.y;
+                }
+#pragma unroll
+                for (int x = 0; x < 4; x++)
+#pragma unroll
+                    for (int y = 0; y < 2; y++) {
+                        fill_dmma884(acc1[x][y], apq[x], br[y]);
+                        fill_dmma884(acc2[x][y], ar[x], bm[y]);
+                        fill_dmma884(acc3[x][y], ai[x], bp[y]);
+                    }
+            }
         }
-        __syncthreads();
-    }
-    // a thread holds two neighbouring outputs (n, n + 1) of a row: 32 contiguous bytes; the 4 lanes of a row write one 128-byte line
+        // a thread holds two neighbouring outputs (n, n + 1) of a row: 32 contiguous bytes; the 4 lanes of a row write one 128-byte line
 #pragma unroll
-    for (int x = 0; x < 4; x++) {
-        const long m = m0 + wm + 8 * x + fr;
-        if (m >= M) continue;
+        for (int x = 0; x < 4; x++) {
+            const long m = m0 + wm + 8 * x + fr;
+            if (m >= M) continue;
 #pragma unroll
-        for (int y = 0; y < 4; y++) {
-            const long n = n0 + wn + 8 * y + 2 * fk;
-            if (n < N) C[m * ldc + n] = make_double2(norm * acc_re[x][y][0], norm * acc_im[x][y][0]);
-            if (n + 1 < N) C[m * ldc + n + 1] = make_double2(norm * acc_re[x][y][1], norm * acc_im[x][y][1]);
+            for (int y = 0; y < 2; y++) {
+                const long n = n0 + wn + 16 * half + 8 * y + 2 * fk;
+                if (n < N) C[m * ldc + n] = make_double2(norm * (acc1[x][y][0] - acc3[x][y][0]), norm * (acc1[x][y][0] + acc2[x][y][0]));
+                if (n + 1 < N) C[m * ldc + n + 1] = make_double2(norm * (acc1[x][y][1] - acc3[x][y][1]), norm * (acc1[x][y][1] + acc2[x][y][1]));
+            }
         }
     }
 }
