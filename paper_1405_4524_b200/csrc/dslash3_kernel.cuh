@@ -194,6 +194,9 @@ template <int K> __device__ __forceinline__ void reduce_scatter_sites(float (&v)
 #ifndef CLV_R3_CBUF
 #define CLV_R3_CBUF 1
 #endif
+#ifndef CLV_R3_LBUF
+#define CLV_R3_LBUF 2
+#endif
 template <int B, int RECON, int XMODE, int PINV, int DOT, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, CLV_R3_CTAS_PER_SM_WARPS * 32 / BLOCK)
 dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, unsigned *__restrict__ sched)
@@ -207,7 +210,8 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
     constexpr int ND = DOT == DOT_XW ? 7 : 3;     // sums per rhs
     constexpr int K = DOT == DOT_XW ? 2 : 1;      // accumulators per thread after the reduce-scatter: values K s .. K s + K - 1 of (2 ND padded to 8 K)
     constexpr int NCB = CLV_R3_CBUF;              // clover buffers
-    __shared__ __align__(128) float lk_s[2][SITES * LREC];
+    constexpr int NLB = CLV_R3_LBUF;              // link buffers
+    __shared__ __align__(128) float lk_s[NLB][SITES * LREC];
     __shared__ __align__(128) float cl_s[NCB][CLOV ? SITES * CREC : 4];
     __shared__ __align__(8) unsigned long long bar[2], bar_c[NCB];
     __shared__ unsigned next_s[2];
@@ -240,14 +244,14 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
         if (CLOV) post_clover(tile, 0);
     }
     do {
-        const int buf = it & 1, cbuf = NCB == 2 ? buf : 0;
-        const unsigned par = (it >> 1) & 1, cpar = NCB == 2 ? par : (it & 1);
+        const int buf = it & 1, cbuf = NCB == 2 ? buf : 0, lbuf = NLB == 2 ? buf : 0;
+        const unsigned par = (it >> 1) & 1, cpar = NCB == 2 ? par : (it & 1), lpar = NLB == 2 ? par : (it & 1);
         if (threadIdx.x == 0) {   // draw the next tile and post its links; buf^1 was released by the barrier that ended iteration it-1
             // (drawing the ticket one tile earlier, so that nobody waits for the atomic, measured 2 % slower)
             const unsigned nt = gridDim.x + atomicAdd(&sched[0], 1u);
             next_s[buf] = nt;
             if (nt < ntiles) {
-                post_links(nt, buf ^ 1);
+                if (NLB == 2) post_links(nt, buf ^ 1);
                 if (CLOV && NCB == 2) post_clover(nt, buf ^ 1);
             }
         }
@@ -274,11 +278,11 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
                 prefetch_l2(q4 + 32 * q);
                 if (q < 2) prefetch_l2(q4 + 32 * (q + 4));
             }
-            const float *rec = &lk_s[buf][site * LREC];
+            const float *rec = &lk_s[lbuf][site * LREC];
             {
                 HopIn2 d;
                 hop_gather3<B, 0, 1>(g, a.in, cb, rhs, c, d);
-                mbar_wait(&bar[buf], par);   // this tile's links have landed (posted one tile ahead)
+                mbar_wait(&bar[lbuf], lpar);   // this tile's links have landed (posted one tile ahead)
 #define CLV_HOP3(MU, FW) lds_link<RECON, 2 * MU + 1 - FW>(rec, d.u); hop_compute2<RECON, MU, FW>(d, hA, hB);
 #define CLV_GAT3(MU, FW) hop_gather3<B, MU, FW>(g, a.in, cb, rhs, c, d);
                 CLV_HOP3(0, 1) CLV_GAT3(0, 0) CLV_HOP3(0, 0) CLV_GAT3(1, 1) CLV_HOP3(1, 1) CLV_GAT3(1, 0) CLV_HOP3(1, 0)
@@ -317,12 +321,15 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
                 }
             }
         } else {
-            mbar_wait(&bar[buf], par);
+            mbar_wait(&bar[lbuf], lpar);
             if (CLOV) mbar_wait(&bar_c[cbuf], cpar);
         }
-        if (CLOV && NCB == 1) {   // the clover buffer has been read: it takes the next tile's blocks while this tile is finished and the next one hops
+        if ((CLOV && NCB == 1) || NLB == 1) {   // the clover buffer has been read: it takes the next tile's blocks while this tile is finished and the next one hops
             __syncthreads();
-            if (threadIdx.x == 0 && next_s[buf] < ntiles) post_clover(next_s[buf], 0);
+            if (threadIdx.x == 0 && next_s[buf] < ntiles) {
+                if (NLB == 1) post_links(next_s[buf], 0);
+                if (CLOV && NCB == 1) post_clover(next_s[buf], 0);
+            }
         }
         if (active) {
             cx<float> wA[12], wB[12];
