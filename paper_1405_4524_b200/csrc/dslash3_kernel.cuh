@@ -87,25 +87,9 @@ __device__ __forceinline__ void hop_gather3(const Geom &g, const float4 *__restr
     d.neg = wrap && g.bc[MU] < 0;
 }
 
-// Own-site streams of the epilogue (x, w): no prefetch.  (The pair kernel prefetches them into L1 at kernel start; here the L1 is smaller
-// by the record buffers and the lines do not survive the hop: measured at 24^3x48, s epilogue 254 us with, 245 us without.)
-#ifndef CLV_R3_PF
-#define CLV_R3_PF 0   // 0 none, 1 prefetch.L1 at tile start, 2 prefetch.L2 at tile start, 3 prefetch.L1 after direction 3
-#endif
+// (Own-site streams of the epilogue, x and w: no prefetch.  The pair kernel prefetches them into L1 at kernel start; here the L1 is smaller by the
+// record buffers and the lines do not survive the hop: measured at 24^3x48, s epilogue 254 us with, 245 us without; into L2: 255 us.)
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-template <int XMODE, int DOT, int LEVEL> __device__ __forceinline__ void prefetch_own_site(const DslashArgs<float> &a, unsigned j)
-{
-    if (XMODE != XM_NONE) {
-        const float4 *q = a.xin + lb_index(j, 0, 6);
-#pragma unroll
-        for (int k = 0; k < 6; k++) { if (LEVEL == 1) prefetch_l1(q + 32 * k); else prefetch_l2(q + 32 * k); }
-    }
-    if (DOT == DOT_W || DOT == DOT_RES || DOT == DOT_S || DOT == DOT_XW) {
-        const float4 *q = a.w + lb_index(j, 0, 6);
-#pragma unroll
-        for (int k = 0; k < 6; k++) { if (LEVEL == 1) prefetch_l1(q + 32 * k); else prefetch_l2(q + 32 * k); }
-    }
-}
 
 // per-tile partial sums of one rhs in fp32 (the 12 terms of a site; same definitions as dots<> in dslash2_kernel.cuh)
 template <int DOT> __device__ __forceinline__ void dots_f(const cx<float> acc[12], const cx<float> x[12], const cx<float> w[12], float *f)
@@ -266,7 +250,6 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
             HopAcc<float> hA, hB;
             hA.zero();
             hB.zero();
-            if (CLV_R3_PF == 1 || CLV_R3_PF == 2) prefetch_own_site<XMODE, DOT, CLV_R3_PF>(a, j);   // x and w lines (the pair shares them)
             if (CLV_R3_PFT) {
                 // Tiles are processed in order of cb (t slowest), so the forward-t neighbours are the frontier: nobody has read them yet
                 // and their gather, the seventh direction, is a DRAM miss.  Ask L2 for their lines now: lane (site, pair q) takes rows
@@ -286,7 +269,6 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
 #define CLV_HOP3(MU, FW) lds_link<RECON, 2 * MU + 1 - FW>(rec, d.u); hop_compute2<RECON, MU, FW>(d, hA, hB);
 #define CLV_GAT3(MU, FW) hop_gather3<B, MU, FW>(g, a.in, cb, rhs, c, d);
                 CLV_HOP3(0, 1) CLV_GAT3(0, 0) CLV_HOP3(0, 0) CLV_GAT3(1, 1) CLV_HOP3(1, 1) CLV_GAT3(1, 0) CLV_HOP3(1, 0)
-                if (CLV_R3_PF == 3) prefetch_own_site<XMODE, DOT, 1>(a, j);
                 CLV_GAT3(2, 1) CLV_HOP3(2, 1) CLV_GAT3(2, 0) CLV_HOP3(2, 0) CLV_GAT3(3, 1) CLV_HOP3(3, 1) CLV_GAT3(3, 0) CLV_HOP3(3, 0)
 #undef CLV_HOP3
 #undef CLV_GAT3

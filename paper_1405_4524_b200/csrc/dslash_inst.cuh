@@ -6,7 +6,6 @@
 #include "dslash3d_kernel.cuh"
 #endif
 #include <algorithm>
-#include <cstdio>
 #include <cstdlib>
 
 namespace clv {
@@ -77,12 +76,6 @@ static int launch_dslash3_BR(const clover_ctx *ctx, const OpData<float> &op, con
             cudaError_t e = cudaFuncGetAttributes(&fa, kern);                                                            \
             if (e != cudaSuccess) return e;                                                                              \
             e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, r3_carveout_pct(fa.sharedSizeBytes, CLV_R3_GRID_PER_SM)); \
-            if (getenv("CLOVER_DEBUG_OCC")) {                                                                            \
-                int occ = -1;                                                                                            \
-                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLK, 0);                                       \
-                fprintf(stderr, "dslash3<%d,%d,%d> smem %zu regs %d carveout %d%% occupancy %d CTAs/SM\n", XM, PI, DT, fa.sharedSizeBytes, fa.numRegs, \
-                        r3_carveout_pct(fa.sharedSizeBytes, CLV_R3_GRID_PER_SM), occ);                                   \
-            }                                                                                                            \
             return e;                                                                                                    \
         }();                                                                                                             \
         CLV_CUDA(attr);                                                                                                  \

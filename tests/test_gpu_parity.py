@@ -66,6 +66,8 @@ ALL_OPS = range(7)
     ((2, 2, 2, 2), (1, 1, 1, -1), 8),       # x+mu == x-mu, padded lane blocks
     ((6, 4, 2, 4), (-1, 1, -1, 1), 5),      # antiperiodic in x and z, Xh odd
     ((8, 8, 8, 16), (1, 1, 1, 1), 8),       # the paper's periodic-in-time choice
+    ((6, 4, 2, 4), (-1, 1, -1, 1), 8),      # the persistent B = 8 kernels on an odd Xh, antiperiodic x and z, Z = 2 (x+mu == x-mu in z)
+    ((4, 6, 8, 10), (1, -1, 1, -1), 8),     # ... and on an anisotropic lattice
 ])
 def test_dslash_ops_fp64_and_fp32(B, dims, bc, n_rhs):
     S = Setup(B, dims, 0.4, 0.118, 1.5, seed=101, bc=bc)
