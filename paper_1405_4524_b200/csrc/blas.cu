@@ -273,17 +273,21 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
     // stage 1: this block sums its contiguous slice of the per-block partials (fixed order); plane 2 only where the step has one
     const int per = (nblocks + SC_SLICES - 1) / SC_SLICES, lo = slice * per, hi = min(nblocks, lo + per);
     double a[7] = {0, 0, 0, 0, 0, 0, 0};
+    // (16-byte loads, four lines in flight per thread: the persistent B = 8 kernels leave one line per tile, 41472 at 24^3x48)
+#pragma unroll 4
     for (int b = lo + threadIdx.x; b < hi; b += 256) {
-        const double *q = partial + ((size_t)b * B + rhs) * 4;
-        a[0] += q[0];
-        a[1] += q[1];
-        a[2] += q[2];
+        const double2 *q = reinterpret_cast<const double2 *>(partial + ((size_t)b * B + rhs) * 4);
+        const double2 q01 = __ldcg(q), q23 = __ldcg(q + 1);
+        a[0] += q01.x;
+        a[1] += q01.y;
+        a[2] += q23.x;
         if (partial2) {
-            const double *q2 = partial2 + ((size_t)b * B + rhs) * 4;
-            a[3] += q2[0];
-            a[4] += q2[1];
-            a[5] += q2[2];
-            a[6] += q2[3];
+            const double2 *q2 = reinterpret_cast<const double2 *>(partial2 + ((size_t)b * B + rhs) * 4);
+            const double2 p01 = __ldcg(q2), p23 = __ldcg(q2 + 1);
+            a[3] += p01.x;
+            a[4] += p01.y;
+            a[5] += p23.x;
+            a[6] += p23.y;
         }
     }
 #pragma unroll
