@@ -114,6 +114,15 @@ int noise_fill(void *out_dev, int precision, const int dims[4], uint64_t seed, i
  * [t][i][j].  fp64 arithmetic, deterministic summation order.  Needs no context; scratch is stream-ordered
  * (cudaMallocAsync).  Asynchronous on `stream`. */
 int stochastic_operators(const double *eta_dev, const double *x_dev, const int dims[4], int n_rhs, double *o_dev, void *stream);
+/* The same O_ij(t) (eq. 7.6) for callers that cannot allocate: code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc.  This call allocates and frees NOTHING (no cudaMalloc / cudaMallocAsync / cudaFree): the per-chunk partial sums go to
+ * a fixed 16 MiB device array inside the library (held by every GPU that loads it, until exit), so the size is limited:
+ * T * n_rhs^2 <= CLOVER_NOALLOC_MAX_TNN, else CLOVER_EINVAL with a message (use stochastic_operators then).  Inputs and output as for
+ * stochastic_operators, caller-owned.  All calls share the array and it keeps the last call's contents (nothing in it needs clearing: every
+ * element read is written first by the same call); calls that OVERLAP on the GPU (two streams, two host threads) race on it -- serialise
+ * them.  Results equal stochastic_operators up to the summation order over k-chunks (1e-13).  Asynchronous on `stream`. */
+#define CLOVER_NOALLOC_MAX_TNN 1048576
+int stochastic_operators_noalloc(const double *eta_dev, const double *x_dev, const int dims[4], int n_rhs, double *o_dev, void *stream);
 /* C(t0, t) = (1 / (n_rhs^2 scale^4)) sum_ij O_ij(t) O_ji(t0)  (eq. 7.7 for every pair of timeslices; scale = the noise scale,
  * R7).  o_dev as above; c_dev: double [T][T][2] (device), index [t0][t].  Asynchronous on `stream`. */
 int stochastic_correlator(const double *o_dev, int T, int n_rhs, double scale, double *c_dev, void *stream);

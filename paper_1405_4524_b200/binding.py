@@ -18,7 +18,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 OP_HOP_EO, OP_HOP_OE, OP_HOP_FULL, OP_CLOVER, OP_CLOVER_INV, OP_D_FULL, OP_MHAT = range(7)
 KERNEL_HOP, KERNEL_AINV_HOP, KERNEL_A_MINUS_HOP, KERNEL_A_MINUS_HOP_S, KERNEL_A_MINUS_HOP_XW = range(5)
 EXPORTS = ["clover_create", "clover_destroy", "dslash_apply", "clover_solve", "clover_solve_host", "noise_fill",
-           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_correlator", "stochastic_fill", "timeslice_norm2", "timeslice_inner"]
+           "clover_bench_kernel", "clover_get_stats", "clover_last_error", "stochastic_operators", "stochastic_operators_noalloc", "stochastic_correlator", "stochastic_fill", "timeslice_norm2", "timeslice_inner"]
 
 
 class ClovOpts(ctypes.Structure):
@@ -50,6 +50,7 @@ _lib.clover_bench_kernel.argtypes = [_vp, _i, _i, _i, _i, _i, ctypes.POINTER(cty
 _lib.clover_get_stats.argtypes = [_vp, ctypes.POINTER(SolveStats)]
 _lib.clover_last_error.argtypes = [_vp]
 _lib.stochastic_operators.argtypes = [_vp, _vp, _ip, _i, _vp, _vp]
+_lib.stochastic_operators_noalloc.argtypes = [_vp, _vp, _ip, _i, _vp, _vp]
 _lib.stochastic_correlator.argtypes = [_vp, _i, _i, _d, _vp, _vp]
 _lib.stochastic_fill.argtypes = [_vp, _vp, _ip, _i, _i, _d, _i, _vp, _vp]
 _lib.timeslice_norm2.argtypes = [_vp, ctypes.c_longlong, _i, ctypes.c_longlong, _vp, _vp]
@@ -107,6 +108,21 @@ def stochastic_operators(eta, x):
     o = torch.empty((T, n, n), dtype=torch.complex128, device="cuda")
     _check(_lib.stochastic_operators(eta.data_ptr(), x.data_ptr(), _i4((X, Y, Z, T)), n, o.data_ptr(), _stream()))
     return o
+
+
+NOALLOC_MAX_TNN = 1048576   # include/clover.h: CLOVER_NOALLOC_MAX_TNN
+
+
+def stochastic_operators_noalloc(eta, x, out):
+    """stochastic_operators without any allocation in the library (fixed internal scratch; T * n^2 <= NOALLOC_MAX_TNN): the caller
+    passes the output `out` complex128 [T, n, n] on the device.  Calls that overlap on the GPU race on the shared scratch."""
+    _require_cuda()
+    assert eta.is_cuda and x.is_cuda and eta.is_contiguous() and x.is_contiguous() and eta.dtype == x.dtype == torch.complex128
+    assert eta.shape == x.shape
+    n, T, Z, Y, X = eta.shape[:5]
+    assert out.is_cuda and out.is_contiguous() and out.dtype == torch.complex128 and tuple(out.shape) == (T, n, n)
+    _check(_lib.stochastic_operators_noalloc(eta.data_ptr(), x.data_ptr(), _i4((X, Y, Z, T)), n, out.data_ptr(), _stream()))
+    return out
 
 
 def stochastic_correlator(o, scale=1.0):

@@ -127,6 +127,20 @@ int stochastic_operators(const double *eta_dev, const double *x_dev, const int d
     return launch_contract(eta_dev, x_dev, dims, n_rhs, o_dev, (cudaStream_t)stream);
 }
 
+int stochastic_operators_noalloc(const double *eta_dev, const double *x_dev, const int dims[4], int n_rhs, double *o_dev, void *stream)
+{
+    if (!eta_dev || !x_dev || !o_dev) { set_error("stochastic_operators_noalloc: null argument"); return CLOVER_EINVAL; }
+    CLV_CHECK(check_dims(dims));
+    if (n_rhs < 1) { set_error("stochastic_operators_noalloc: n_rhs = %d must be >= 1", n_rhs); return CLOVER_EINVAL; }
+    if ((long long)dims[3] * n_rhs * n_rhs > CLOVER_NOALLOC_MAX_TNN) {
+        set_error("stochastic_operators_noalloc: T * n_rhs^2 = %lld exceeds CLOVER_NOALLOC_MAX_TNN = %d (use stochastic_operators)",
+                  (long long)dims[3] * n_rhs * n_rhs, CLOVER_NOALLOC_MAX_TNN);
+        return CLOVER_EINVAL;
+    }
+    CLV_CHECK(check_device());
+    return launch_contract_noalloc(eta_dev, x_dev, dims, n_rhs, o_dev, (cudaStream_t)stream);
+}
+
 int stochastic_correlator(const double *o_dev, int T, int n_rhs, double scale, double *c_dev, void *stream)
 {
     if (!o_dev || !c_dev) { set_error("stochastic_correlator: null argument"); return CLOVER_EINVAL; }

@@ -112,6 +112,7 @@ int launch_noise(void *out, int precision, const int dims[4], uint64_t seed, int
 
 // ---- contract.cu ----
 int launch_contract(const double *eta, const double *xs, const int dims[4], int n, double *o, cudaStream_t st);
+int launch_contract_noalloc(const double *eta, const double *xs, const int dims[4], int n, double *o, cudaStream_t st);
 int launch_correlator(const double *o, int T, int n, double scale, double *c, cudaStream_t st);
 
 // ---- fill.cu ----

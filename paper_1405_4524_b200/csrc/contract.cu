@@ -10,6 +10,7 @@
 #include "context.h"
 #include <algorithm>
 #include <cuda_pipeline.h>
+#include <mutex>
 
 namespace clv {
 
@@ -165,6 +166,63 @@ int launch_contract(const double *eta, const double *xs, const int dims[4], int 
     contract_reduce_kernel<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(partial, count, (int)nch, (double2 *)o);
     CLV_CUDA(cudaGetLastError());
     CLV_CUDA(cudaFreeAsync(partial, st));
+    return 0;
+}
+
+// ---- allocation-free variant of launch_contract (include/clover.h: stochastic_operators_noalloc) -----------------------------------
+// For callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the per-chunk
+// partial sums live in this fixed array instead of a cudaMallocAsync block.  Every GPU that loads the library holds its 16 MiB until exit.
+// In host code `ct_noalloc_scratch` is only the host-side stand-in of the symbol, NOT a device address: the device address is taken with
+// cudaGetSymbolAddress once per device (with that device current) and that pointer is what the kernels get.
+// All calls share the array and it keeps the last call's contents.  Nothing in it has to start at zero: every element of the
+// [nch][T][n][n] block that contract_reduce_kernel reads is written first by contract_kernel of the same call (every k-chunk is non-empty
+// and every (t, tile) CTA stores its whole tile), so no clear is issued.  Two calls that overlap on the GPU (different streams, or two
+// host threads) race on the array: callers serialise them.
+constexpr long CT_NOALLOC_MAX = 1L << 20;   // complex numbers (CLOVER_NOALLOC_MAX_TNN in clover.h): T * n_rhs^2 * chunks must fit
+static __device__ __align__(256) double2 ct_noalloc_scratch[CT_NOALLOC_MAX];
+
+static int noalloc_scratch_ptr(double2 **out)
+{
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static double2 *ptr[MAX_DEV] = {};
+    int dev = -1;
+    CLV_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) { set_error("stochastic_operators_noalloc: device ordinal %d out of range", dev); return CLOVER_EINVAL; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void *q = nullptr;
+        CLV_CUDA(cudaGetSymbolAddress(&q, ct_noalloc_scratch));   // device `dev` is current: this is ITS copy of the array
+        ptr[dev] = static_cast<double2 *>(q);
+    }
+    *out = ptr[dev];
+    return 0;
+}
+
+int launch_contract_noalloc(const double *eta, const double *xs, const int dims[4], int n, double *o, cudaStream_t st)
+{
+    const int T = dims[3];
+    const long K = 12L * dims[0] * dims[1] * dims[2];
+    const int tiles = (n + CT_TILE - 1) / CT_TILE;
+    const long count = (long)T * n * n;
+    if (count > CT_NOALLOC_MAX) {
+        set_error("stochastic_operators_noalloc: T * n_rhs^2 = %ld exceeds the fixed scratch of %ld complex numbers (use stochastic_operators)", count,
+                  CT_NOALLOC_MAX);
+        return CLOVER_EINVAL;
+    }
+    // k-chunks as in launch_contract, but no more than the scratch holds
+    long nch = std::max<long>(1, (10L * 148 + (long)T * tiles * tiles - 1) / ((long)T * tiles * tiles));
+    nch = std::min<long>(nch, std::max<long>(1, K / (8 * CT_KT)));
+    nch = std::min<long>(nch, CT_NOALLOC_MAX / count);
+    long kchunk = (K + nch - 1) / nch;
+    kchunk = (kchunk + CT_KT - 1) / CT_KT * CT_KT;
+    nch = (K + kchunk - 1) / kchunk;
+    double2 *partial = nullptr;
+    CLV_CHECK(noalloc_scratch_ptr(&partial));
+    contract_kernel<<<dim3((unsigned)nch, T, tiles * tiles), CT_THREADS, 0, st>>>((const double2 *)eta, (const double2 *)xs, n, T, K, kchunk, tiles, partial);
+    CLV_CUDA(cudaGetLastError());
+    contract_reduce_kernel<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(partial, count, (int)nch, (double2 *)o);
+    CLV_CUDA(cudaGetLastError());
     return 0;
 }
 
