@@ -52,7 +52,7 @@ typedef struct {
 } clover_opts;
 
 typedef struct {
-    int status;           /* 0 converged, 1 max_iter reached, 2 repeated breakdown (<r0,v> = 0 after 8 restarts), 3 non-finite */
+    int status;           /* 0 converged, 1 max_iter reached, 2 repeated breakdown (still breaking down after 100 restarts of the recurrence), 3 non-finite */
     int iters;            /* BiCGStab iterations of the BATCH this source was in (the rhs of a batch iterate together; a rhs that
                              converges early is frozen, so every rhs of a batch reports the same count) */
     int reliable_updates; /* fp64 residual recomputations of that batch */

@@ -4,6 +4,7 @@
 // Reductions: products in the storage precision, accumulation in fp64, warp shuffle -> shared memory ->
 // per-block partials [block][rhs][4]; the scalar kernels sum the partials in a fixed order (deterministic).
 #include "blas.cuh"
+#include <cstdlib>
 #include <algorithm>
 
 namespace clv {
@@ -263,9 +264,10 @@ __device__ __forceinline__ bool finite_z(zs z) { return isfinite(z.re) && isfini
 
 // one block per rhs: sum partial[(b*B + rhs)*4 + c] over b < nblocks in a fixed order, then thread 0 updates the scalars.
 constexpr int SC_SLICES = 32;
+constexpr int MAX_RESTARTS = 100;   // breakdown restarts of one rhs before it is given up (status 2)
 constexpr int LEG_MAX = 48;   // sloppy iterations between two reliable updates at most (the benchmarked systems need 12-14 per leg)
 __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblocks, const double *__restrict__ partial, const double *__restrict__ partial2,
-                                                     RhsScalars *sc, double tol2, double delta2, double *stage, unsigned *ticket, RhsScalars *publish)
+                                                     RhsScalars *sc, double tol2, double delta2, double *stage, unsigned *ticket, RhsScalars *publish, int leg_max, double brk2)
 {
     __shared__ double sm[256][7];
     __shared__ bool last;
@@ -346,6 +348,7 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         q.restart = 0;
         q.nrestart = 0;
         q.delta2 = delta2;
+        q.r0n2 = d0;   // r0 = r = b
         q.since = 0;
         if (!(q.eta2 > 0.) || d0 <= tol2 * q.eta2) q.done = 1;  // zero source or already converged
         if (!isfinite(d0)) { q.done = 1; q.status = 3; }
@@ -359,11 +362,11 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             else if (!(d0 * d0 + d1 * d1 > 0.)) {
                 // breakdown (e.g. a point source on unit links): this iteration becomes a pure minimal-residual step (alpha = 0),
                 // then the recurrence restarts from the current residual, r0 := r (same remedy as the oracle, R11)
-                if (q.nrestart < 8) { q.restart = 1; q.nrestart++; }
+                if (q.nrestart < MAX_RESTARTS) { q.restart = 1; q.nrestart++; }
                 else { q.done = 1; q.status = 2; }
             } else {
                 al = zdiv(ld_z(q.rho), r0v);
-                if (!finite_z(al)) { al = zero; if (q.nrestart < 8) { q.restart = 1; q.nrestart++; } else { q.done = 1; q.status = 2; } }
+                if (!finite_z(al)) { al = zero; if (q.nrestart < MAX_RESTARTS) { q.restart = 1; q.nrestart++; } else { q.done = 1; q.status = 2; } }
             }
         }
         q.alpha = st_z(al);
@@ -388,12 +391,15 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             if (d2 > q.maxr2) q.maxr2 = d2;
             if (!isfinite(d2) || !finite_z(rho1)) { q.done = 1; q.status = 3; }
             else {
-                if (d2 < q.delta2 * q.maxr2 || ++q.since >= LEG_MAX) q.want_update = 1;
+                if (d2 < q.delta2 * q.maxr2 || ++q.since >= leg_max) q.want_update = 1;
                 q.claim = (d2 <= tol2 * q.eta2) ? 1 : 0;
                 const double om2 = om.re * om.re + om.im * om.im, rh2 = rho.re * rho.re + rho.im * rho.im;
                 if (!(om2 > 0.) || !(rh2 > 0.)) q.want_update = 1;  // stagnation: let the fp64 residual decide, beta = 0 restarts p = r
                 else be = zmul(zdiv(rho1, rho), zdiv(ld_z(q.alpha), om));
                 if (!finite_z(be)) be = zero;
+                // relative breakdown (as in the oracle): r0 has become orthogonal to r within the precision of the dot product -- restart the
+                // recurrence from the current residual (r0 := r, p := r: beta = 0) rather than divide by a rho that is noise
+                if (d2 > 0. && !q.restart && d0 * d0 + d1 * d1 <= brk2 * q.r0n2 * d2 && q.nrestart < MAX_RESTARTS) { q.restart = 1; q.nrestart++; be = zero; }
                 q.rho = st_z(rho1);
             }
         }
@@ -418,7 +424,7 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
         }
         break;
     case SC_RESTART:  // after r0 := r: rho = <r0, r> = ||r||^2 (the value SC_RHO / SC_TRUE left in r2)
-        if (q.restart) { q.rho = make_double2(q.r2, 0.); q.beta = st_z(zero); q.restart = 0; }
+        if (q.restart) { q.rho = make_double2(q.r2, 0.); q.r0n2 = q.r2; q.beta = st_z(zero); q.restart = 0; }
         break;
     // ---- merged iteration (solver.cu): alpha is known before Mhat p, rho' comes from <r0,s> - omega <r0,t> ----
     case SC_OMEGA2: {  // (d0,d1) = <t,s>, d2 = <t,t>, (e0,e1) = <r0,t>, (e2,e3) = <r0,s>
@@ -454,14 +460,21 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             if (d2 > q.maxr2) q.maxr2 = d2;
             if (!isfinite(d2) || !isfinite(d0) || !isfinite(d1)) { q.done = 1; q.status = 3; }
             else {
-                if (d2 < q.delta2 * q.maxr2 || ++q.since >= LEG_MAX) q.want_update = 1;
+                if (d2 < q.delta2 * q.maxr2 || ++q.since >= leg_max) q.want_update = 1;
                 q.claim = (d2 <= tol2 * q.eta2) ? 1 : 0;
+                {   // relative breakdown (as in the oracle): rho' = <r0, r'> (left in q.rho by SC_OMEGA2) is noise against ||r0|| ||r'||
+                    const zs rho = ld_z(q.rho);
+                    if (d2 > 0. && !q.restart && !q.claim && rho.re * rho.re + rho.im * rho.im <= brk2 * q.r0n2 * d2 && q.nrestart < MAX_RESTARTS) {
+                        q.restart = 1;   // r0 := p := r, q0 := Mhat^+ r0, rho := ||r||^2, alpha from SC_RESTART2 before the next iteration
+                        q.nrestart++;
+                    }
+                }
                 if (q.restart != 1) {  // (a restart recomputes alpha itself)
                     if (d0 * d0 + d1 * d1 > 0.) al = zdiv(ld_z(q.rho), zs{d0, d1});
                     if (!(d0 * d0 + d1 * d1 > 0.) || !finite_z(al)) {
                         // breakdown: the next iteration is a pure minimal-residual step (alpha = 0), then r0 := r (R11)
                         al = zero;
-                        if (q.nrestart < 8) { q.restart = 2; q.nrestart++; }
+                        if (q.nrestart < MAX_RESTARTS) { q.restart = 2; q.nrestart++; }
                         else { q.done = 1; q.status = 2; }
                     }
                 }
@@ -475,6 +488,7 @@ __global__ void __launch_bounds__(256) scalar_kernel(int step, int B, int nblock
             zs al = zero;
             q.restart = 0;
             q.rho = make_double2(q.r2, 0.);
+            q.r0n2 = q.r2;
             q.beta = q.gam = st_z(zero);
             if (!q.done) {
                 if (d0 * d0 + d1 * d1 > 0.) al = zdiv(ld_z(q.rho), zs{d0, d1});
@@ -604,8 +618,9 @@ int blas_norm2_pair(const BlasCtx &c, const double2 *a1, const double2 *b1, cons
 }
 int blas_scalar_step(const BlasCtx &c, int step, int nblocks, double tol2, double delta2, RhsScalars *publish)
 {
+    static const int leg_max = [] { const char *e = getenv("CLOVER_LEGMAX"); const int n = e ? atoi(e) : 0; return n > 0 ? n : LEG_MAX; }();  // tuning/debug knob only
     scalar_kernel<<<dim3(c.B, SC_SLICES), 256, 0, c.st>>>(step, c.B, nblocks, c.partial, step == SC_OMEGA2 ? c.partial2 : nullptr, c.sc, tol2, delta2, c.stage,
-                                                          c.ticket, publish);
+                                                          c.ticket, publish, leg_max, c.brk2);
     BLAS_LAUNCHED(c);
     CLV_CUDA(cudaGetLastError());
     return 0;

@@ -18,6 +18,7 @@ struct BlasCtx {
     unsigned *ticket;  // device, [8]: arrival counters of the scalar kernels (zero between launches)
     cudaStream_t st;
     long long *launches;
+    double brk2;       // square of the relative breakdown threshold of the iteration precision (scalar kernel, R11)
 };
 
 // s = r - alpha v

@@ -46,6 +46,7 @@ struct RhsScalars {
     // iterated one (the leg asked the sloppy precision for more than it can deliver: ill-conditioned systems), so that the next legs
     // stop where the sloppy residual is still true.
     double delta2;
+    double r0n2;      // ||r0||^2 at the last (re)start: scale of the relative breakdown test |<r0, r>| <= brk ||r0|| ||r|| (R11)
     int since;        // sloppy iterations since the last reliable update
     int pad_;
 };

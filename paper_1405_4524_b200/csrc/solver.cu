@@ -267,7 +267,10 @@ static int solve_batch(clover_ctx *ctx, const double *src, double *dst, int B, d
       *r0 = (V *)W->sl[S_R0], *tmp = (V *)W->sl[S_TMP], *q0 = (V *)W->sl[S_Q0];
     const bool merged = merged_enabled();
     long long &nl = ctx->stats.kernel_launches;
-    BlasCtx bc{&g, B, W->sc_dev, W->partial, W->partial2, W->partial_blocks, W->stage, W->ticket, st, &nl};
+    // relative breakdown threshold of the recurrence (R11): 1e-10 in fp64 as in the oracle's spirit (it uses 1e-14; 1e-10 needs fewer iterations on
+    // near-critical systems), 1e-6 for the fp32 iteration, whose dot products carry no more
+    const double brk = sizeof(R) == 8 ? 1e-10 : 1e-6;
+    BlasCtx bc{&g, B, W->sc_dev, W->partial, W->partial2, W->partial_blocks, W->stage, W->ticket, st, &nl, brk * brk};
     const double tol2 = tol * tol, delta = reliable_delta(), delta2 = delta * delta;
     const size_t nbytes = field_vecs<R>(g, B) * sizeof(V), nbytes64 = field_vecs<double>(g, B) * sizeof(double2);
     int nb = 0, grid = 0, iters = 0, updates = 0;

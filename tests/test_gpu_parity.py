@@ -281,14 +281,18 @@ def test_dslash_apply_is_asynchronous_on_its_stream(B):
     S.ctx.close()
 
 
-@pytest.mark.parametrize("dims,eps", [((4, 4, 4, 8), 0.4), ((8, 8, 8, 16), 0.4), ((8, 8, 8, 16), 0.5)])
+@pytest.mark.parametrize("dims,eps", [((4, 4, 4, 8), 0.4), ((8, 8, 8, 16), 0.4), ((8, 8, 8, 16), 0.5), ((4, 4, 4, 8), 0.3), ((8, 8, 8, 16), 0.3)])
 def test_solve_at_the_papers_parameter_point(B, dims, eps):
     """The paper's own point: kappa = 0.13514 (m0 a = -0.300), c_sw = 1.0, periodic in all four directions, on rough
     synthetic links, 8 sources, mixed precision.  These systems are far worse conditioned than BASELINE.json's (hundreds of
     iterations instead of 25): the fp32 legs cannot deliver the solver's default delta, so this is the test that the reliable
     updates (adaptive per-rhs delta, R11) still converge to 1e-10 and that the result is the oracle's.  With
     cond(D) ~ 1e3 a residual of 1e-10 bounds the solution error only by ~1e-7, so the 1e-8 solution bar is checked on a solve to
-    1e-12 (both sides), and the 1e-10 solve is held to cond(D) * residual with the oracle-solved solution as the reference."""
+    1e-12 (both sides), and the 1e-10 solve is held to cond(D) * residual with the oracle-solved solution as the reference.
+    eps = 0.3 is near-critical at this kappa: BiCGStab without a RELATIVE breakdown test (restart with r0 := p := r when |<r0, r>| is noise
+    against ||r0|| ||r||, as the oracle has it) does not converge there at all -- neither on the GPU (before the test was added to the
+    scalar kernel) nor as a plain numpy recurrence, even-odd or not; with it the even-odd solve needs 420-850 iterations (the oracle,
+    unpreconditioned: 940-1750)."""
     kappa, csw, bc = 0.13514, 1.0, (1, 1, 1, 1)
     S = Setup(B, dims, eps, kappa, csw, seed=77, bc=bc)
     eta = B.noise_fill(dims, 5, 8, scale=wl.INV_SQRT2)
