@@ -99,3 +99,29 @@ def test_cfg4_32x32x32x64_recon12_dilution():
     # first and last batch of the 64 time-diluted sources (timeslices 0..7 and 56..63); oracle solves: source 0 and the source on
     # timeslice 63
     _run(4, [(0, 8), (56, 8)], oracle_solved=(0, 63))
+
+
+def test_cfg3_solve_host_matches_device_path():
+    """clover_solve_host at the bench configuration (32 sources, batch 8, copies overlapped with the solves; the call bench.py's e2e times):
+    every source converges, sources of the first, a middle and the last batch get the oracle's residual, and all 32 solutions are the
+    device-buffer path's bit for bit (same batches, same kernels, same order)."""
+    from paper_1405_4524_b200 import binding as B
+    c = wl.CONFIGS[3]
+    dims, kappa = c["dims"], c["kappa"]
+    U = wl.gauge_links(dims, c["eps"], c["gauge_seed"])
+    A = oracle.clover_matrix(U, kappa, c["csw"])
+    ctx = B.Clover(torch.from_numpy(U).cuda(), kappa, c["csw"], bc=wl.BC, recon=c["recon"], max_rhs=8)
+    eta = B.noise_fill(dims, c["noise_seed"], c["n_rhs"], scale=wl.INV_SQRT2)
+    psi_dev, infos_dev, bad = ctx.solve(eta, tol=wl.TOL, batch=8, mixed=True)
+    assert bad == 0
+    h_eta = eta.cpu().pin_memory()
+    h_psi = torch.empty_like(h_eta).pin_memory()
+    _, infos, bad = ctx.solve_host(h_eta, tol=wl.TOL, batch=8, mixed=True, out=h_psi)
+    assert bad == 0, infos
+    assert all(i["status"] == 0 and i["true_resid"] <= wl.TOL for i in infos)
+    e, p = h_eta.numpy(), h_psi.numpy()
+    for r in (0, 7, 12, 31):
+        res = _oracle_residual(U, A, kappa, e[r], p[r])
+        assert res <= wl.TOL and abs(infos[r]["true_resid"] - res) <= 1e-3 * res + 1e-14, (r, res, infos[r])
+    assert torch.equal(h_psi, psi_dev.cpu()) and infos == infos_dev
+    ctx.close()
