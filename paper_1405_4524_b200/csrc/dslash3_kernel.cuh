@@ -91,6 +91,75 @@ __device__ __forceinline__ void hop_gather3(const Geom &g, const float4 *__restr
 // record buffers and the lines do not survive the hop: measured at 24^3x48, s epilogue 254 us with, 245 us without; into L2: 255 us.)
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// yA (+)= M xA, yB (+)= M xB for the two packed 6x6 Hermitian blocks of a site (rows `srow` in shared memory), on the packed f32x2 pipe: the two
+// right-hand sides of the thread ride in the two halves of an FFMA2 and the matrix element is its broadcast operand, so the 504 flop of a
+// clover product cost 126 FFMA2 + 12 FMUL2 per rhs pair instead of 480 FFMA + 24 FMUL (a three-register FFMA and an FFMA2 hold the FP32 pipe equally long).
+#ifndef CLV_R3_CLOVER_PACKED
+#define CLV_R3_CLOVER_PACKED 1
+#endif
+template <bool ACCUM>
+__device__ __forceinline__ void clover_mul2_packed(const float4 *srow, const cx<float> xA[12], cx<float> yA[12], const cx<float> xB[12], cx<float> yB[12])
+{
+#pragma unroll
+    for (int blk = 0; blk < 2; blk++) {
+        const int o = 6 * blk;
+        cx<float> m[18];
+#pragma unroll
+        for (int k = 0; k < 9; k++) {
+            const float4 v = srow[9 * blk + k];
+            m[2 * k] = mk<float>(v.x, v.y);
+            m[2 * k + 1] = mk<float>(v.z, v.w);
+        }
+        float2 xr[6], xi[6], yr[6], yi[6];
+#pragma unroll
+        for (int i = 0; i < 6; i++) {
+            xr[i] = make_float2(xA[o + i].re, xB[o + i].re);
+            xi[i] = make_float2(xA[o + i].im, xB[o + i].im);
+            if (ACCUM) {
+                yr[i] = make_float2(yA[o + i].re, yB[o + i].re);
+                yi[i] = make_float2(yA[o + i].im, yB[o + i].im);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 3; k++) {   // real diagonal entries (2k, 2k) = m[k].re and (2k+1, 2k+1) = m[k].im
+            const float2 d0 = make_float2(m[k].re, m[k].re), d1 = make_float2(m[k].im, m[k].im);
+            if (ACCUM) {
+                yr[2 * k] = __ffma2_rn(d0, xr[2 * k], yr[2 * k]);
+                yi[2 * k] = __ffma2_rn(d0, xi[2 * k], yi[2 * k]);
+                yr[2 * k + 1] = __ffma2_rn(d1, xr[2 * k + 1], yr[2 * k + 1]);
+                yi[2 * k + 1] = __ffma2_rn(d1, xi[2 * k + 1], yi[2 * k + 1]);
+            } else {
+                yr[2 * k] = __fmul2_rn(d0, xr[2 * k]);
+                yi[2 * k] = __fmul2_rn(d0, xi[2 * k]);
+                yr[2 * k + 1] = __fmul2_rn(d1, xr[2 * k + 1]);
+                yi[2 * k + 1] = __fmul2_rn(d1, xi[2 * k + 1]);
+            }
+        }
+        int k = 3;
+#pragma unroll
+        for (int i = 1; i < 6; i++)
+#pragma unroll
+            for (int j = 0; j < i; j++, k++) {
+                const float2 mr = make_float2(m[k].re, m[k].re), mi = make_float2(m[k].im, m[k].im), nmi = make_float2(-m[k].im, -m[k].im);
+                // y[i] += m x[j]
+                yr[i] = __ffma2_rn(mr, xr[j], yr[i]);
+                yr[i] = __ffma2_rn(nmi, xi[j], yr[i]);
+                yi[i] = __ffma2_rn(mr, xi[j], yi[i]);
+                yi[i] = __ffma2_rn(mi, xr[j], yi[i]);
+                // y[j] += conj(m) x[i]
+                yr[j] = __ffma2_rn(mr, xr[i], yr[j]);
+                yr[j] = __ffma2_rn(mi, xi[i], yr[j]);
+                yi[j] = __ffma2_rn(mr, xi[i], yi[j]);
+                yi[j] = __ffma2_rn(nmi, xr[i], yi[j]);
+            }
+#pragma unroll
+        for (int i = 0; i < 6; i++) {
+            yA[o + i] = mk<float>(yr[i].x, yi[i].x);
+            yB[o + i] = mk<float>(yr[i].y, yi[i].y);
+        }
+    }
+}
+
 // per-tile partial sums of one rhs in fp32 (the 12 terms of a site; same definitions as dots<> in dslash2_kernel.cuh)
 template <int DOT> __device__ __forceinline__ void dots_f(const cx<float> acc[12], const cx<float> x[12], const cx<float> w[12], float *f)
 {
@@ -291,10 +360,12 @@ dslash3_kernel(const Geom g, const OpData<float> op, const DslashArgs<float> a, 
             if (CLOV) {
                 mbar_wait(&bar_c[cbuf], cpar);
                 const float4 *srow = reinterpret_cast<const float4 *>(&cl_s[cbuf][site * CREC]);
+                // (packed form for the A^-1 product only: measured at 24^3x48, A^-1 H 176 -> 170 us; for y += A x it costs more moves than it saves: +3-5 %)
                 if (XMODE == XM_CLOVER) clover_mul2<true>(nullptr, cb, srow, xA, accA, xB, accB);
                 if (PINV) {
                     cx<float> tA[12], tB[12];
-                    clover_mul2<false>(nullptr, cb, srow, accA, tA, accB, tB);
+                    if (CLV_R3_CLOVER_PACKED) clover_mul2_packed<false>(srow, accA, tA, accB, tB);
+                    else clover_mul2<false>(nullptr, cb, srow, accA, tA, accB, tB);
 #pragma unroll
                     for (int i = 0; i < 12; i++) {
                         accA[i] = tA[i];
