@@ -39,7 +39,7 @@ def test_noalloc_matches_existing_path_on_consecutive_calls():
         free_before = torch.cuda.mem_get_info()[0]
         got = B.stochastic_operators_noalloc(eta, x, out)
         torch.cuda.synchronize()
-        assert torch.cuda.mem_get_info()[0] == free_before                  # the call took no device memory
+        assert torch.cuda.mem_get_info()[0] >= free_before                  # the call took no device memory (a pool may have released some)
         got = got.cpu().numpy()
         assert np.isfinite(got).all() and nerr(got, want) < TOL, (k, nerr(got, want))
         if k == 0:
